@@ -1,0 +1,67 @@
+"""Seeded synthetic initial conditions and the BASELINE.json workload table.
+
+This module is the ONLY code shared by the CUDA path and the CPU oracle.  It
+holds none of the method's arithmetic: it only draws the i.i.d. uniform initial
+fields C0 = cbar + A*U(-1,1) ("r(x) is a random number drawn
+from the uniform random distribution ... independent identical distributions";
+amplitudes/means are the BASELINE.json configs')
+and names the five workload shapes.
+
+Generator (G9): counter based, so value j of member seed s does not depend on
+the order of generation:  z = splitmix64_finalise(s * GOLDEN + (j + 1) * GAMMA2),
+U = 2 * (z >> 11) * 2**-53 - 1, flat index j x-fastest.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+_GOLDEN = np.uint64(0x9E3779B97F4A7C15)
+_GAMMA2 = np.uint64(0xD1B54A32D192ED03)
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+
+
+def uniform_pm1(seed: int, count: int) -> np.ndarray:
+    """`count` i.i.d. U(-1,1) doubles for member seed `seed` (order independent)."""
+    with np.errstate(over="ignore"):
+        j = np.arange(1, count + 1, dtype=np.uint64)
+        z = np.uint64(seed) * _GOLDEN + j * _GAMMA2
+        z = (z ^ (z >> np.uint64(30))) * _M1
+        z = (z ^ (z >> np.uint64(27))) * _M2
+        z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) * (2.0 ** -52) - 1.0
+
+
+def initial_state(seeds, N: int, D: int, cbar, amp: float) -> np.ndarray:
+    """C0[m][(z)][y][x] = cbar_m + amp * U(-1,1), one seed per member."""
+    seeds = list(seeds)
+    cbars = [float(cbar)] * len(seeds) if np.isscalar(cbar) else [float(c) for c in cbar]
+    assert len(cbars) == len(seeds)
+    out = np.empty((len(seeds),) + (N,) * D, dtype=np.float64)
+    for m, (s, cb) in enumerate(zip(seeds, cbars)):
+        out[m] = cb + amp * uniform_pm1(s, N ** D).reshape((N,) * D)
+    return out
+
+
+# BASELINE.json configs (index = position in `configs`): h = 1, gamma = 1, dt = 0.01.
+CONFIGS = {
+    "cfg1": dict(ensemble=1, N=64, D=2, gamma=1.0, dt=0.01, nsteps=5000, stride=10,
+                 cbar=0.0, amp=0.1, seed0=0),
+    "cfg2": dict(ensemble=64, N=256, D=2, gamma=1.0, dt=0.01, nsteps=20000, stride=50,
+                 cbar=0.0, amp=0.05, seed0=1000),
+    "cfg3": dict(ensemble=128, N=512, D=2, gamma=1.0, dt=0.01, nsteps=20000, stride=50,
+                 cbar=-0.4, amp=0.05, seed0=2000),
+    "cfg4": dict(ensemble=16, N=128, D=3, gamma=1.0, dt=0.01, nsteps=10000, stride=50,
+                 cbar=[0.0] * 8 + [-0.4] * 8, amp=0.05, seed0=3000),
+    "cfg5": dict(ensemble=8, N=2048, D=2, gamma=1.0, dt=0.01, nsteps=5000, stride=50,
+                 cbar=-0.2, amp=0.05, seed0=4000),
+}
+
+
+def config_state(name: str, members=None) -> np.ndarray:
+    """Initial ensemble of a named config; `members` selects a subset of member indices."""
+    c = CONFIGS[name]
+    idx = list(range(c["ensemble"])) if members is None else list(members)
+    cb = c["cbar"]
+    cbars = [cb[k] for k in idx] if isinstance(cb, (list, tuple)) else [cb] * len(idx)
+    return initial_state([c["seed0"] + k for k in idx], c["N"], c["D"], cbars, c["amp"])
