@@ -1,0 +1,142 @@
+/*
+ * ch.h -- C ABI of libch: ensemble Cahn-Hilliard semi-implicit ADI stepper for
+ * NVIDIA B200 (sm_100a), fp64, one GPU per context.
+ *
+ * Citations: P:nnn = line nnn of the paper text (arXiv 1911.03386, PAPER.md);
+ * Gk = reading k in DESIGN.md ("Readings of the paper").
+ *
+ * The method (eq.(3); "semi-implicit ADI finite-difference
+ * method, periodic boundary conditions"; scheme left open by the paper and fixed by
+ * reading G1/G2).  Grid spacing h = 1, periodic N^D grid per ensemble member:
+ *
+ *     mu^n    = (C^n)^3 - C^n - gamma Lap_h C^n
+ *     r       = dt Lap_h mu^n
+ *     w       = A_z^-1 A_y^-1 A_x^-1 r       A_d = I + gamma dt (delta_d^2)^2, cyclic pentadiagonal,
+ *                                            rows (s,-4s,1+6s,-4s,s), s = gamma dt; A_z only if D = 3
+ *     C^{n+1} = C^n + w
+ *
+ * which is (I + s dxx^2)(I + s dyy^2) C^{n+1} = C^n + dt Lap_h[(C^n)^3 - C^n]
+ * - 2 s dxx dyy C^n + s^2 dxx^2 dyy^2 C^n  (three factors in 3D) with C^n subtracted
+ * from both sides.  Diagnostics of a state at time t (eq.(4) with the bulk
+ * prefactor 1/4, G3; forward differences, G4; eq.(6); eq.(43)):
+ *
+ *     F    = sum_i [ (C_i^2 - 1)^2 / 4 + gamma/2 sum_d (C_{i+e_d} - C_i)^2 ]
+ *     Fdot = - sum_i sum_d (mu_{i+e_d} - mu_i)^2
+ *     mass = sum_i C_i
+ *     beta = - t Fdot / F                    (0 when F == 0)
+ *
+ * A physical run with spacing h maps onto h = 1 by gamma' = gamma/h^2, dt' = dt/h^2,
+ * F = h^D F', beta unchanged.
+ *
+ * Layout: every state / field pointer is ensemble * N^D contiguous doubles,
+ * C[m][y][x] (D = 2) or C[m][z][y][x] (D = 3), x fastest, member stride N^D.
+ * "on_device" arguments say whether a caller pointer is device (1) or host (0) memory.
+ *
+ * Ownership: the context owns its factorisation tables and, unless a workspace is
+ * attached, its device arrays.  State passed in or out is copied.  A series buffer
+ * is caller-owned device memory and must outlive every ch_step that writes it.
+ *
+ * Errors: every call returns CH_OK (0) or a negative code; nothing throws or aborts
+ * across the boundary.  ch_last_error() gives a message for the last failure on a
+ * context.  There is no CPU fallback: without a CUDA device ch_create fails with
+ * CH_ECUDA.
+ *
+ * Determinism: same inputs give bitwise-same outputs run to run; the result of a
+ * member does not depend on the ensemble size or on its position in the ensemble.
+ */
+#ifndef CH_H
+#define CH_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ch_ctx ch_ctx;   /* opaque; created by ch_create, freed by ch_destroy */
+
+enum {
+    CH_OK = 0,
+    CH_EINVAL = -1,      /* null pointer, ensemble < 1, D not in {2,3}, N < 8, gamma <= 0, dt <= 0,
+                            nsteps < 0, workspace too small, series full, unknown option */
+    CH_ENOMEM = -2,      /* host or device allocation failed */
+    CH_ECUDA = -3,       /* CUDA runtime error (message in ch_last_error) */
+    CH_ESTATE = -4,      /* step / energy / get_state before set_state */
+    CH_ENONFINITE = -5   /* ch_energy found a non-finite F (state has blown up) */
+};
+
+/* Create a context for `ensemble` independent members on an N^D periodic grid (D = 2 or 3,
+ * N >= 8, any N; N a multiple of 16 takes the fast kernels) with parameters gamma, dt of
+ * eq.(3) at h = 1.  Computes the periodic (circulant) LU factorisation of A_d on the host
+ * (DESIGN.md "Factorisation").  Uses the current CUDA device.  *out is set on success. */
+int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma, double dt);
+
+/* Free the context and everything it owns (not an attached workspace, not the series). */
+int ch_destroy(ch_ctx *ctx);
+
+/* Stream on which every later call enqueues its work (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream).  Default: the legacy default stream. */
+int ch_set_stream(ch_ctx *ctx, void *cuda_stream);
+
+/* Bytes of device memory a context of this shape needs (state, work array, reduction
+ * partials).  0 on invalid arguments. */
+size_t ch_workspace_bytes(int ensemble, int N, int D);
+
+/* Use caller-owned device memory (256-byte aligned, >= ch_workspace_bytes) instead of
+ * cudaMalloc.  Must be called before ch_set_state; the buffer must outlive the context. */
+int ch_attach_workspace(ch_ctx *ctx, void *dev, size_t bytes);
+
+/* Copy ensemble*N^D doubles into the context (stream-ordered; synchronises if the source
+ * is host memory).  Resets the step counter n = 0, the time origin t0 = 0 and the series cursor. */
+int ch_set_state(ch_ctx *ctx, const double *C, int on_device);
+
+/* Time origin for beta after a restart: samples are taken at t = t0 + n dt (G6). */
+int ch_set_time(ch_ctx *ctx, double t0);
+
+/* Per-member time series, caller-owned DEVICE buffer series[capacity][ensemble][4] =
+ * {F, dF/dt, beta, mass}.  A sample is written for the state after n steps whenever
+ * n % stride == 0, including n = 0 (sample k at t = t0 + k stride dt).
+ * Pass NULL to switch sampling off.  Resets the series cursor. */
+int ch_set_series(ch_ctx *ctx, double *series_dev, int stride, int capacity);
+
+/* Advance every member by nsteps steps.  Asynchronous: work is enqueued on the stream and
+ * the call returns.  CH_EINVAL (nothing enqueued) if the series would overflow. */
+int ch_step(ch_ctx *ctx, int nsteps);
+
+/* {F, dF/dt, beta, mass} of the current state, out[ensemble][4].  With a host pointer the
+ * call synchronises the stream and returns CH_ENONFINITE if any F is not finite. */
+int ch_energy(ch_ctx *ctx, double *out, int on_device);
+
+/* Copy the current state out (stream-ordered; synchronises if the target is host memory). */
+int ch_get_state(ch_ctx *ctx, double *C, int on_device);
+
+/* Number of series samples written (enqueued) so far, steps taken since ch_set_state. */
+int ch_series_count(const ch_ctx *ctx);
+long long ch_step_count(const ch_ctx *ctx);
+
+/* Components of one step, exported for per-kernel parity tests and profiling.
+ * ch_rhs:   r = dt Lap_h mu(C) of the CURRENT state into r_out (device or host).
+ * ch_sweep: w := A_axis^-1 w on a caller field of the context's shape (axis 0 = x, 1 = y, 2 = z),
+ *           in place, device or host.  Neither touches the state or the step counter. */
+int ch_rhs(ch_ctx *ctx, double *r_out, int on_device);
+int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
+
+/* Kernel-variant and launch options (measurement knobs; every variant computes the same step):
+ *   "graph"      0/1   replay one sampling period as a CUDA graph (default 1)
+ *   "sweep"      0     auto, 1 force the generic thread-per-line sweeps, 2 force the chunked sweeps
+ *   "fuse_rhs_x" 0/1   fuse the RHS stencil into the x-sweep kernel where supported (default 1)
+ *   "batch"      k     advance k members at a time through a whole sampling period so that
+ *                      their state stays L2-resident (0 = whole ensemble per launch)          */
+int ch_set_option(ch_ctx *ctx, const char *key, int value);
+int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
+
+/* Kernel launches enqueued by this context since creation (each graph node counts once per replay). */
+long long ch_launch_count(const ch_ctx *ctx);
+
+/* Message for the last error on this context (never NULL); ch_create failures: pass NULL. */
+const char *ch_last_error(const ch_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CH_H */

@@ -1,0 +1,237 @@
+"""Thin ctypes binding over the C ABI of include/ch.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libch.so; there is no CPU fallback:
+loading fails loudly if the library has not been built (python -m paper_1911_03386_b200.build),
+and ch_create fails without a CUDA device.  Module-level functions carry the C names;
+`Ensemble` is a convenience wrapper holding the context.  Arrays may be numpy (host)
+or torch CUDA tensors (device); torch is used only for device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+CH_OK, CH_EINVAL, CH_ENOMEM, CH_ECUDA, CH_ESTATE, CH_ENONFINITE = 0, -1, -2, -3, -4, -5
+
+EXPORTS = [
+    "ch_create", "ch_destroy", "ch_set_stream", "ch_workspace_bytes", "ch_attach_workspace",
+    "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_energy", "ch_get_state",
+    "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
+    "ch_launch_count", "ch_last_error",
+]
+
+_LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libch.so")
+_lib = None
+
+
+class ChError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libch error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libch.so (raises if it is missing: the CUDA path is the only path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise RuntimeError(f"{_LIBPATH} not built; run `python -m paper_1911_03386_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(_LIBPATH)
+        vp, dp, ci, cd = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        L.ch_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cd, cd]
+        L.ch_destroy.argtypes = [vp]
+        L.ch_set_stream.argtypes = [vp, vp]
+        L.ch_workspace_bytes.argtypes = [ci, ci, ci]
+        L.ch_workspace_bytes.restype = ctypes.c_size_t
+        L.ch_attach_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+        L.ch_set_state.argtypes = [vp, dp, ci]
+        L.ch_set_time.argtypes = [vp, cd]
+        L.ch_set_series.argtypes = [vp, dp, ci, ci]
+        L.ch_step.argtypes = [vp, ci]
+        L.ch_energy.argtypes = [vp, dp, ci]
+        L.ch_get_state.argtypes = [vp, dp, ci]
+        L.ch_series_count.argtypes = [vp]
+        L.ch_step_count.argtypes = [vp]
+        L.ch_step_count.restype = ctypes.c_longlong
+        L.ch_rhs.argtypes = [vp, dp, ci]
+        L.ch_sweep.argtypes = [vp, dp, ci, ci]
+        L.ch_set_option.argtypes = [vp, ctypes.c_char_p, ci]
+        L.ch_get_option.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ci)]
+        L.ch_launch_count.argtypes = [vp]
+        L.ch_launch_count.restype = ctypes.c_longlong
+        L.ch_last_error.argtypes = [vp]
+        L.ch_last_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    """(address, on_device) of a C-contiguous float64 numpy array or torch tensor."""
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+        return a.ctypes.data, 0
+    import torch
+    assert isinstance(a, torch.Tensor) and a.dtype == torch.float64 and a.is_contiguous()
+    return a.data_ptr(), 1 if a.is_cuda else 0
+
+
+def _check(ctx, rc):
+    if rc != CH_OK:
+        raise ChError(rc, lib().ch_last_error(ctx).decode())
+
+
+# ---- C names ---------------------------------------------------------------------------
+def ch_create(ensemble, N, D, gamma, dt):
+    ctx = ctypes.c_void_p()
+    rc = lib().ch_create(ctypes.byref(ctx), ensemble, N, D, gamma, dt)
+    if rc != CH_OK:
+        raise ChError(rc, lib().ch_last_error(None).decode())
+    return ctx
+
+
+def ch_destroy(ctx):
+    return lib().ch_destroy(ctx)
+
+
+def ch_set_stream(ctx, stream):
+    _check(ctx, lib().ch_set_stream(ctx, ctypes.c_void_p(stream)))
+
+
+def ch_workspace_bytes(ensemble, N, D):
+    return lib().ch_workspace_bytes(ensemble, N, D)
+
+
+def ch_attach_workspace(ctx, tensor):
+    _check(ctx, lib().ch_attach_workspace(ctx, tensor.data_ptr(), tensor.numel() * tensor.element_size()))
+
+
+def ch_set_state(ctx, C):
+    p, dev = _ptr(C)
+    _check(ctx, lib().ch_set_state(ctx, p, dev))
+
+
+def ch_set_time(ctx, t0):
+    _check(ctx, lib().ch_set_time(ctx, t0))
+
+
+def ch_set_series(ctx, series, stride, capacity):
+    _check(ctx, lib().ch_set_series(ctx, None if series is None else series.data_ptr(), stride, capacity))
+
+
+def ch_step(ctx, nsteps):
+    _check(ctx, lib().ch_step(ctx, nsteps))
+
+
+def ch_energy(ctx, out):
+    p, dev = _ptr(out)
+    _check(ctx, lib().ch_energy(ctx, p, dev))
+
+
+def ch_get_state(ctx, C):
+    p, dev = _ptr(C)
+    _check(ctx, lib().ch_get_state(ctx, p, dev))
+
+
+def ch_series_count(ctx):
+    return lib().ch_series_count(ctx)
+
+
+def ch_step_count(ctx):
+    return lib().ch_step_count(ctx)
+
+
+def ch_rhs(ctx, r_out):
+    p, dev = _ptr(r_out)
+    _check(ctx, lib().ch_rhs(ctx, p, dev))
+
+
+def ch_sweep(ctx, w, axis):
+    p, dev = _ptr(w)
+    _check(ctx, lib().ch_sweep(ctx, p, axis, dev))
+
+
+def ch_set_option(ctx, key, value):
+    _check(ctx, lib().ch_set_option(ctx, key.encode(), int(value)))
+
+
+def ch_get_option(ctx, key):
+    v = ctypes.c_int()
+    rc = lib().ch_get_option(ctx, key.encode(), ctypes.byref(v))
+    if rc != CH_OK:
+        raise ChError(rc, f"unknown option {key}")
+    return v.value
+
+
+def ch_launch_count(ctx):
+    return lib().ch_launch_count(ctx)
+
+
+# ---- convenience wrapper ---------------------------------------------------------------
+class Ensemble:
+    """Context holder: Ensemble(ensemble, N, D, gamma, dt); methods mirror the C calls."""
+
+    def __init__(self, ensemble, N, D, gamma, dt, stream=None, options=None):
+        self.shape = (ensemble,) + (N,) * D
+        self.ensemble, self.N, self.D, self.gamma, self.dt = ensemble, N, D, gamma, dt
+        self.ctx = ch_create(ensemble, N, D, gamma, dt)
+        self._series = None
+        self.stride = 0
+        if stream is not None:
+            ch_set_stream(self.ctx, stream)
+        for k, v in (options or {}).items():
+            ch_set_option(self.ctx, k, v)
+
+    def close(self):
+        if self.ctx is not None:
+            ch_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, C):
+        assert tuple(C.shape) == self.shape, (tuple(C.shape), self.shape)
+        ch_set_state(self.ctx, C)
+
+    def set_series(self, stride, capacity):
+        """Allocate a device series buffer [capacity][ensemble][4] (torch) and register it."""
+        import torch
+        self._series = torch.zeros((capacity, self.ensemble, 4), dtype=torch.float64, device="cuda")
+        self.stride = stride
+        ch_set_series(self.ctx, self._series, stride, capacity)
+
+    def step(self, nsteps):
+        ch_step(self.ctx, nsteps)
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty(self.shape, dtype=np.float64)
+        ch_get_state(self.ctx, out)
+        return out
+
+    def energy(self):
+        out = np.empty((self.ensemble, 4), dtype=np.float64)
+        ch_energy(self.ctx, out)
+        return out
+
+    def series(self):
+        """Samples written so far, as a host array [count][ensemble][4]."""
+        import torch
+        torch.cuda.synchronize()
+        return self._series[: ch_series_count(self.ctx)].cpu().numpy()
+
+    def rhs(self):
+        out = np.empty(self.shape, dtype=np.float64)
+        ch_rhs(self.ctx, out)
+        return out
+
+    def sweep(self, w, axis):
+        w = np.array(w, dtype=np.float64, order="C", copy=True)
+        ch_sweep(self.ctx, w, axis)
+        return w

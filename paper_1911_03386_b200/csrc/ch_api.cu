@@ -1,0 +1,461 @@
+// ch_api.cu -- the C ABI of include/ch.h: argument checking, host precompute, workspace,
+// kernel selection and launch.  No torch types, no exceptions across the boundary.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/ch.h"
+#include "ch_factor.h"
+#include "ch_kernels.cuh"
+
+struct ch_ctx {
+    int M, N, D;
+    double gamma, dt;
+    size_t npts;            // N^D
+    size_t total;           // M * N^D
+    bool pow2;
+    // factorisation
+    ChFactor fac;
+    bool chunked;           // chunked sweeps available for this N
+    int LC;
+    double *dW;             // device copy of fac.W
+    double rscale;          // dt / c0^D: the 1/c0 of every sweep folded into the RHS
+    // device arrays
+    void *ws_base;          // cudaMalloc'ed or attached
+    bool ws_owned;
+    size_t ws_bytes;
+    double *C, *w, *partials, *eout;
+    int nparts;             // RHS tiles per member
+    int rhs_tiles_x, rhs_tiles_y;
+    // state
+    bool has_state;
+    long long n;            // steps since set_state
+    double t0;
+    double *series;
+    int stride, capacity, cursor;
+    long long last_sampled; // step index whose sample has been written (-1: none)
+    cudaStream_t stream;
+    // options
+    int opt_sweep;          // 0 auto, 1 generic, 2 chunked
+    long long launches;
+    std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(ch_ctx *ctx, int code, const std::string &msg)
+{
+    if (ctx) ctx->err = msg; else g_create_err = msg;
+    return code;
+}
+
+#define CUDA_TRY(ctx, call)                                                                         \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(ctx, CH_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+    } while (0)
+
+static size_t ipow(size_t n, int d) { size_t p = 1; while (d-- > 0) p *= n; return p; }
+static size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+static int rhs_parts(int N, int D)
+{
+    if (D == 2) return ((N + RHS2_TX - 1) / RHS2_TX) * ((N + RHS2_TY - 1) / RHS2_TY);
+    return ((N + RHS3_TX - 1) / RHS3_TX) * ((N + RHS3_TY - 1) / RHS3_TY) * ((N + RHS3_TZ - 1) / RHS3_TZ);
+}
+
+static bool shape_ok(int ensemble, int N, int D) { return ensemble >= 1 && N >= 8 && (D == 2 || D == 3); }
+
+extern "C" size_t ch_workspace_bytes(int ensemble, int N, int D)
+{
+    if (!shape_ok(ensemble, N, D)) return 0;
+    const size_t total = (size_t)ensemble * ipow(N, D);
+    return 2 * align256(total * 8) + align256((size_t)ensemble * rhs_parts(N, D) * 3 * 8) + align256((size_t)ensemble * 4 * 8);
+}
+
+static void carve(ch_ctx *c)
+{
+    char *p = (char *)c->ws_base;
+    c->C = (double *)p; p += align256(c->total * 8);
+    c->w = (double *)p; p += align256(c->total * 8);
+    c->partials = (double *)p; p += align256((size_t)c->M * c->nparts * 3 * 8);
+    c->eout = (double *)p;
+}
+
+static int chunk_len_for(int N)
+{
+    if (N % 16 != 0 || N < 16) return 0;
+    if (N / 16 <= 64) return 16;
+    if (N % 32 == 0 && N / 32 <= CH_MAX_P) return 32;
+    return 0;
+}
+
+extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma, double dt)
+{
+    if (!out) return fail(nullptr, CH_EINVAL, "ch_create: out is NULL");
+    *out = nullptr;
+    if (!shape_ok(ensemble, N, D)) return fail(nullptr, CH_EINVAL, "ch_create: need ensemble >= 1, N >= 8, D in {2,3}");
+    if (!(gamma > 0) || !(dt > 0) || !std::isfinite(gamma) || !std::isfinite(dt))
+        return fail(nullptr, CH_EINVAL, "ch_create: need finite gamma > 0 and dt > 0");
+    if (ipow(N, D) * (size_t)ensemble > ((size_t)1 << 40)) return fail(nullptr, CH_EINVAL, "ch_create: problem too large");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, CH_ECUDA, "ch_create: no CUDA device (libch has no CPU fallback)");
+    }
+    ch_ctx *c = new (std::nothrow) ch_ctx();
+    if (!c) return fail(nullptr, CH_ENOMEM, "ch_create: out of host memory");
+    c->M = ensemble; c->N = N; c->D = D; c->gamma = gamma; c->dt = dt;
+    c->npts = ipow(N, D); c->total = c->npts * ensemble;
+    c->pow2 = (N & (N - 1)) == 0;
+    c->LC = chunk_len_for(N);
+    c->chunked = c->LC != 0;
+    if (ch_factor_build(&c->fac, N, gamma * dt, c->LC) != 0) {
+        delete c;
+        return fail(nullptr, CH_EINVAL, "ch_create: factorisation of I + gamma dt (delta^2)^2 failed its self-check");
+    }
+    c->rscale = dt / std::pow(c->fac.c0, D);
+    c->dW = nullptr;
+    c->nparts = rhs_parts(N, D);
+    if (D == 2) { c->rhs_tiles_x = (N + RHS2_TX - 1) / RHS2_TX; c->rhs_tiles_y = (N + RHS2_TY - 1) / RHS2_TY; }
+    else { c->rhs_tiles_x = (N + RHS3_TX - 1) / RHS3_TX; c->rhs_tiles_y = (N + RHS3_TY - 1) / RHS3_TY; }
+    c->ws_base = nullptr; c->ws_owned = false; c->ws_bytes = 0;
+    c->C = c->w = c->partials = c->eout = nullptr;
+    c->has_state = false; c->n = 0; c->t0 = 0.0;
+    c->series = nullptr; c->stride = 0; c->capacity = 0; c->cursor = 0; c->last_sampled = -1;
+    c->stream = 0; c->opt_sweep = 0; c->launches = 0;
+    if (c->chunked) {
+        cudaError_t e = cudaMalloc((void **)&c->dW, sizeof(double) * 4 * CH_MAX_P);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dW, c->fac.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            std::string msg = std::string("ch_create: ") + cudaGetErrorString(e);
+            if (c->dW) cudaFree(c->dW);
+            delete c;
+            return fail(nullptr, e == cudaErrorMemoryAllocation ? CH_ENOMEM : CH_ECUDA, msg);
+        }
+    }
+    // opt in to the dynamic shared memory the kernels need
+    cudaFuncSetAttribute(k_rhs3d<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_rhs3d<true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_rhs3d<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_rhs3d<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_rhs3d<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_rhs3d<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_sweep_contig<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaFuncSetAttribute(k_sweep_contig<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaFuncSetAttribute(k_sweep_contig<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaFuncSetAttribute(k_sweep_contig<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaGetLastError();
+    *out = c;
+    return CH_OK;
+}
+
+extern "C" int ch_destroy(ch_ctx *ctx)
+{
+    if (!ctx) return CH_EINVAL;
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->ws_owned && ctx->ws_base) cudaFree(ctx->ws_base);
+    if (ctx->dW) cudaFree(ctx->dW);
+    delete ctx;
+    return CH_OK;
+}
+
+extern "C" const char *ch_last_error(const ch_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int ch_set_stream(ch_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return CH_EINVAL;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return CH_OK;
+}
+
+extern "C" int ch_attach_workspace(ch_ctx *ctx, void *dev, size_t bytes)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!dev || ((uintptr_t)dev & 255)) return fail(ctx, CH_EINVAL, "ch_attach_workspace: need a 256-byte aligned device pointer");
+    if (bytes < ch_workspace_bytes(ctx->M, ctx->N, ctx->D)) return fail(ctx, CH_EINVAL, "ch_attach_workspace: workspace too small");
+    if (ctx->has_state) return fail(ctx, CH_ESTATE, "ch_attach_workspace: must precede ch_set_state");
+    if (ctx->ws_owned && ctx->ws_base) cudaFree(ctx->ws_base);
+    ctx->ws_base = dev; ctx->ws_owned = false; ctx->ws_bytes = bytes;
+    carve(ctx);
+    return CH_OK;
+}
+
+static int ensure_workspace(ch_ctx *ctx)
+{
+    if (ctx->ws_base) return CH_OK;
+    const size_t bytes = ch_workspace_bytes(ctx->M, ctx->N, ctx->D);
+    cudaError_t e = cudaMalloc(&ctx->ws_base, bytes);
+    if (e != cudaSuccess) {
+        ctx->ws_base = nullptr;
+        cudaGetLastError();
+        return fail(ctx, e == cudaErrorMemoryAllocation ? CH_ENOMEM : CH_ECUDA, std::string("cudaMalloc workspace: ") + cudaGetErrorString(e));
+    }
+    ctx->ws_owned = true; ctx->ws_bytes = bytes;
+    carve(ctx);
+    return CH_OK;
+}
+
+extern "C" int ch_set_state(ch_ctx *ctx, const double *C, int on_device)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!C) return fail(ctx, CH_EINVAL, "ch_set_state: C is NULL");
+    int rc = ensure_workspace(ctx);
+    if (rc) return rc;
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->C, C, ctx->total * 8, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    if (!on_device) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->has_state = true; ctx->n = 0; ctx->t0 = 0.0; ctx->cursor = 0; ctx->last_sampled = -1;
+    return CH_OK;
+}
+
+extern "C" int ch_set_time(ch_ctx *ctx, double t0)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!std::isfinite(t0)) return fail(ctx, CH_EINVAL, "ch_set_time: t0 not finite");
+    ctx->t0 = t0;
+    return CH_OK;
+}
+
+extern "C" int ch_set_series(ch_ctx *ctx, double *series_dev, int stride, int capacity)
+{
+    if (!ctx) return CH_EINVAL;
+    if (series_dev && (stride < 1 || capacity < 1)) return fail(ctx, CH_EINVAL, "ch_set_series: need stride >= 1 and capacity >= 1");
+    ctx->series = series_dev; ctx->stride = series_dev ? stride : 0; ctx->capacity = series_dev ? capacity : 0;
+    ctx->cursor = 0; ctx->last_sampled = -1;
+    return CH_OK;
+}
+
+extern "C" int ch_series_count(const ch_ctx *ctx) { return ctx ? ctx->cursor : CH_EINVAL; }
+extern "C" long long ch_step_count(const ch_ctx *ctx) { return ctx ? ctx->n : CH_EINVAL; }
+extern "C" long long ch_launch_count(const ch_ctx *ctx) { return ctx ? ctx->launches : CH_EINVAL; }
+
+extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
+{
+    if (!ctx || !key) return CH_EINVAL;
+    if (!strcmp(key, "sweep")) {
+        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: sweep must be 0, 1 or 2");
+        if (value == 2 && !ctx->chunked) return fail(ctx, CH_EINVAL, "ch_set_option: chunked sweeps need N % 16 == 0");
+        ctx->opt_sweep = value;
+        return CH_OK;
+    }
+    return fail(ctx, CH_EINVAL, std::string("ch_set_option: unknown option ") + key);
+}
+
+extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
+{
+    if (!ctx || !key || !value) return CH_EINVAL;
+    if (!strcmp(key, "sweep")) { *value = ctx->opt_sweep; return CH_OK; }
+    if (!strcmp(key, "chunked")) { *value = ctx->chunked ? ctx->LC : 0; return CH_OK; }
+    if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
+    return CH_EINVAL;
+}
+
+// ---------------------------------------------------------------------------------------
+// launches
+// ---------------------------------------------------------------------------------------
+template <bool DIAG, bool WRITE>
+static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
+{
+    if (c->D == 2) {
+        dim3 grid(c->nparts, c->M);
+        if (c->pow2) k_rhs2d<DIAG, WRITE, true><<<grid, 256, 0, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x);
+        else k_rhs2d<DIAG, WRITE, false><<<grid, 256, 0, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x);
+    } else {
+        dim3 grid(c->nparts, c->M);
+        if (c->pow2) k_rhs3d<DIAG, WRITE, true><<<grid, 256, RHS3_SMEM, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x, c->rhs_tiles_y);
+        else k_rhs3d<DIAG, WRITE, false><<<grid, 256, RHS3_SMEM, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x, c->rhs_tiles_y);
+    }
+    c->launches++;
+}
+
+static void launch_rhs(ch_ctx *c, const double *C, double *r, double scale, bool diag, bool write)
+{
+    if (diag && write) launch_rhs_t<true, true>(c, C, r, scale);
+    else if (diag) launch_rhs_t<true, false>(c, C, r, scale);
+    else launch_rhs_t<false, true>(c, C, r, scale);
+}
+
+static void launch_finish(ch_ctx *c, double *out, double t)
+{
+    k_finish<<<c->M, 128, 0, c->stream>>>(c->partials, c->nparts, out, t);
+    c->launches++;
+}
+
+static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
+{
+    p.np = c->fac.np; p.nq = c->fac.nq; p.oscale = oscale;
+    memcpy(p.alpha, c->fac.alpha, sizeof(p.alpha));
+    memcpy(p.beta, c->fac.beta, sizeof(p.beta));
+    p.W = c->dW; p.K = c->fac.K; p.P = c->fac.P;
+}
+
+// axis 0 = x, 1 = y, 2 = z.  update: C += result (last sweep of a step).  scale: multiply the output by oscale.
+static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale, double oscale)
+{
+    const int N = c->N, D = c->D, M = c->M;
+    const size_t n2 = (size_t)N * N, n3 = n2 * N;
+    const bool chunked = c->chunked && c->opt_sweep != 1;
+    if (!chunked) {
+        long long n_lines = (long long)M * (D == 3 ? n2 : (size_t)N);
+        int n_inner; size_t os, is, ls;
+        if (axis == 0) { n_inner = 1; os = N; is = 0; ls = 1; }
+        else if (axis == 1) { n_inner = N; os = n2; is = 1; ls = N; }
+        else { n_inner = (int)n2; os = n3; is = 1; ls = n2; }
+        const int blocks = (int)((n_lines + 127) / 128);
+        const double *Wl = c->fac.Wline;
+        if (update) k_sweep_generic<true><<<blocks, 128, 0, c->stream>>>(c->fac.np, c->fac.nq, Wl[0], Wl[1], Wl[2], Wl[3], scale ? oscale : 1.0, w, c->C, N, n_lines, n_inner, os, is, ls);
+        else k_sweep_generic<false><<<blocks, 128, 0, c->stream>>>(c->fac.np, c->fac.nq, Wl[0], Wl[1], Wl[2], Wl[3], scale ? oscale : 1.0, w, c->C, N, n_lines, n_inner, os, is, ls);
+        c->launches++;
+        return;
+    }
+    SweepParams prm;
+    fill_params(c, prm, oscale);
+    const int LC = c->LC, P = c->fac.P;
+    if (axis == 0) {
+        const long long total_lines = (long long)M * (D == 3 ? n2 : (size_t)N);
+        int threads = 256;
+        if (P > threads) threads = P;
+        int LPB = threads / P;
+        if (LPB > total_lines) LPB = (int)total_lines;
+        threads = LPB * P;
+        const int blocks = (int)((total_lines + LPB - 1) / LPB);
+        const size_t smem = (size_t)LPB * N * 8 + (size_t)2 * LPB * P * 8;
+        if (LC == 16) {
+            if (scale) k_sweep_contig<16, true><<<blocks, threads, smem, c->stream>>>(prm, w, N, total_lines, LPB);
+            else k_sweep_contig<16, false><<<blocks, threads, smem, c->stream>>>(prm, w, N, total_lines, LPB);
+        } else {
+            if (scale) k_sweep_contig<32, true><<<blocks, threads, smem, c->stream>>>(prm, w, N, total_lines, LPB);
+            else k_sweep_contig<32, false><<<blocks, threads, smem, c->stream>>>(prm, w, N, total_lines, LPB);
+        }
+        c->launches++;
+        return;
+    }
+    // strided
+    size_t outer_stride, line_stride; int n_inner; long long n_outer;
+    if (axis == 1) { n_inner = N; n_outer = (long long)M * (D == 3 ? N : 1); outer_stride = n2; line_stride = N; }
+    else { n_inner = (int)n2; n_outer = M; outer_stride = n3; line_stride = n2; }
+    int cols = 16;
+    while (cols * P > 512 && cols > 4) cols >>= 1;
+    const int inner_blocks = n_inner / cols;
+    dim3 block(cols, P);
+    const unsigned blocks = (unsigned)(inner_blocks * n_outer);
+    const size_t smem = (size_t)2 * P * cols * 8;
+#define LAUNCH_STRIDED(LCV)                                                                                                          \
+    do {                                                                                                                             \
+        if (update) k_sweep_strided<LCV, true, false><<<blocks, block, smem, c->stream>>>(prm, w, c->C, outer_stride, line_stride, inner_blocks); \
+        else if (scale) k_sweep_strided<LCV, false, true><<<blocks, block, smem, c->stream>>>(prm, w, c->C, outer_stride, line_stride, inner_blocks); \
+        else k_sweep_strided<LCV, false, false><<<blocks, block, smem, c->stream>>>(prm, w, c->C, outer_stride, line_stride, inner_blocks); \
+    } while (0)
+    if (LC == 16) LAUNCH_STRIDED(16); else LAUNCH_STRIDED(32);
+#undef LAUNCH_STRIDED
+    c->launches++;
+}
+
+static int check_launch(ch_ctx *ctx, const char *what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(ctx, CH_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    return CH_OK;
+}
+
+extern "C" int ch_step(ch_ctx *ctx, int nsteps)
+{
+    if (!ctx) return CH_EINVAL;
+    if (nsteps < 0) return fail(ctx, CH_EINVAL, "ch_step: nsteps < 0");
+    if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_step: no state (call ch_set_state first)");
+    if (ctx->series) {
+        // samples this call will write: every n in [n0, n0 + nsteps] with n % stride == 0, not yet sampled
+        long long n0 = ctx->n, n1 = ctx->n + nsteps, cnt = 0;
+        long long first = ((n0 + ctx->stride - 1) / ctx->stride) * ctx->stride;
+        if (first <= n1) cnt = (n1 - first) / ctx->stride + 1;
+        if (first == ctx->last_sampled) cnt -= 1;
+        if (ctx->cursor + cnt > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_step: series full");
+    }
+    const int D = ctx->D;
+    for (int s = 0; s < nsteps; ++s) {
+        const bool sample = ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n;
+        launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
+        if (sample) {
+            launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt);
+            ctx->cursor++; ctx->last_sampled = ctx->n;
+        }
+        for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
+        ctx->n++;
+    }
+    if (ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n) {
+        launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, true, false);
+        launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt);
+        ctx->cursor++; ctx->last_sampled = ctx->n;
+    }
+    return check_launch(ctx, "ch_step");
+}
+
+extern "C" int ch_energy(ch_ctx *ctx, double *out, int on_device)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!out) return fail(ctx, CH_EINVAL, "ch_energy: out is NULL");
+    if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_energy: no state");
+    const double t = ctx->t0 + (double)ctx->n * ctx->dt;
+    launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, true, false);
+    launch_finish(ctx, on_device ? out : ctx->eout, t);
+    int rc = check_launch(ctx, "ch_energy");
+    if (rc) return rc;
+    if (!on_device) {
+        CUDA_TRY(ctx, cudaMemcpyAsync(out, ctx->eout, (size_t)ctx->M * 32, cudaMemcpyDeviceToHost, ctx->stream));
+        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        for (int m = 0; m < ctx->M; ++m)
+            if (!std::isfinite(out[4 * m])) return fail(ctx, CH_ENONFINITE, "ch_energy: non-finite free energy");
+    }
+    return CH_OK;
+}
+
+extern "C" int ch_get_state(ch_ctx *ctx, double *C, int on_device)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!C) return fail(ctx, CH_EINVAL, "ch_get_state: C is NULL");
+    if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_get_state: no state");
+    CUDA_TRY(ctx, cudaMemcpyAsync(C, ctx->C, ctx->total * 8, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    if (!on_device) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    return CH_OK;
+}
+
+extern "C" int ch_rhs(ch_ctx *ctx, double *r_out, int on_device)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!r_out) return fail(ctx, CH_EINVAL, "ch_rhs: r_out is NULL");
+    if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_rhs: no state");
+    double *dst = on_device ? r_out : ctx->w;
+    launch_rhs(ctx, ctx->C, dst, ctx->dt, false, true);
+    int rc = check_launch(ctx, "ch_rhs");
+    if (rc) return rc;
+    if (!on_device) {
+        CUDA_TRY(ctx, cudaMemcpyAsync(r_out, ctx->w, ctx->total * 8, cudaMemcpyDeviceToHost, ctx->stream));
+        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    return CH_OK;
+}
+
+extern "C" int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!w) return fail(ctx, CH_EINVAL, "ch_sweep: w is NULL");
+    if (axis < 0 || axis >= ctx->D) return fail(ctx, CH_EINVAL, "ch_sweep: axis out of range");
+    int rc = ensure_workspace(ctx);
+    if (rc) return rc;
+    double *buf = w;
+    if (!on_device) {
+        buf = ctx->w;
+        CUDA_TRY(ctx, cudaMemcpyAsync(buf, w, ctx->total * 8, cudaMemcpyHostToDevice, ctx->stream));
+    }
+    launch_sweep(ctx, buf, axis, false, true, 1.0 / ctx->fac.c0);
+    rc = check_launch(ctx, "ch_sweep");
+    if (rc) return rc;
+    if (!on_device) {
+        CUDA_TRY(ctx, cudaMemcpyAsync(w, buf, ctx->total * 8, cudaMemcpyDeviceToHost, ctx->stream));
+        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    return CH_OK;
+}

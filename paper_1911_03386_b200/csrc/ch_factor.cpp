@@ -1,0 +1,107 @@
+// ch_factor.cpp -- see ch_factor.h.  Host only; long double throughout, rounded once.
+#include "ch_factor.h"
+
+#include <cmath>
+#include <complex>
+#include <cstring>
+
+namespace {
+
+typedef long double ld;
+
+struct M2 { ld a, b, c, d; };   // [[a b],[c d]]
+
+M2 mul(const M2 &x, const M2 &y)
+{
+    return { x.a * y.a + x.b * y.c, x.a * y.b + x.b * y.d, x.c * y.a + x.d * y.c, x.c * y.b + x.d * y.d };
+}
+
+ld maxabs(const M2 &x) { return fmaxl(fmaxl(fabsl(x.a), fabsl(x.b)), fmaxl(fabsl(x.c), fabsl(x.d))); }
+
+// (I - X)^-1
+M2 inv_i_minus(const M2 &x)
+{
+    ld a = 1 - x.a, b = -x.b, c = -x.c, d = 1 - x.d, det = a * d - b * c;
+    return { d / det, -b / det, -c / det, a / det };
+}
+
+// transfer matrix over n points: [[alpha_{n-1}, beta_{n-1}],[alpha_{n-2}, beta_{n-2}]]
+M2 transfer(ld np, ld nq, int n, ld *alpha, ld *beta)
+{
+    ld a1 = 1, a2 = 0, b1 = 0, b2 = 1;     // u_{-1}, u_{-2}
+    for (int k = 0; k < n; ++k) {
+        ld a = np * a1 + nq * a2, b = np * b1 + nq * b2;
+        if (alpha) { alpha[k] = a; beta[k] = b; }
+        a2 = a1; a1 = a; b2 = b1; b1 = b;
+    }
+    return { a1, b1, a2, b2 };
+}
+
+}  // namespace
+
+int ch_factor_build(ChFactor *f, int N, double sigma, int LC)
+{
+    std::memset(f, 0, sizeof(*f));
+    if (!(sigma > 0) || N < 5 || LC < 0 || LC > CH_MAX_LC) return -1;
+    f->sigma = sigma;
+    // roots of z + 1/z = 2 + i / sqrt(s): the inside pair is z, conj(z)
+    std::complex<ld> w(2.0L, 1.0L / sqrtl((ld)sigma));
+    std::complex<ld> sq = std::sqrt(w * w - (ld)4);
+    std::complex<ld> z = (ld)2 / (w + sq);
+    if (std::abs(z) >= 1) z = (ld)2 / (w - sq);
+    if (!(std::abs(z) < 1)) return -1;
+    ld p = -2 * z.real(), q = std::norm(z), c0 = (ld)sigma / q;
+    // polish (p, q) by Newton on  c0 (1+p^2+q^2) = 1+6s,  c0 p (1+q) = -4s  with c0 = s/q
+    for (int it = 0; it < 3; ++it) {
+        ld s = sigma;
+        ld f1 = s * (1 + p * p + q * q) - (1 + 6 * s) * q;      // multiplied through by q
+        ld f2 = p * (1 + q) + 4 * q;                            // divided by s, multiplied by q
+        ld j11 = 2 * s * p, j12 = 2 * s * q - (1 + 6 * s), j21 = 1 + q, j22 = p + 4;
+        ld det = j11 * j22 - j12 * j21;
+        if (det == 0) break;
+        p -= (f1 * j22 - f2 * j12) / det;
+        q -= (j11 * f2 - j21 * f1) / det;
+    }
+    c0 = (ld)sigma / q;
+    // self-check of the three symbol coefficients
+    ld e0 = fabsl(c0 * (1 + p * p + q * q) - (1 + 6 * (ld)sigma)) / (1 + 6 * (ld)sigma);
+    ld e1 = fabsl(c0 * p * (1 + q) + 4 * (ld)sigma) / (4 * (ld)sigma);
+    if (!(e0 < 1e-15L && e1 < 1e-15L) || !(q < 1)) return -1;
+    f->np = (double)-p; f->nq = (double)-q; f->c0 = (double)c0; f->rho = (double)sqrtl(q);
+    // the tables are built from the ROUNDED coefficients, so that they are the exact
+    // homogeneous solutions of the recurrence the kernels run
+    ld np = f->np, nq = f->nq;
+
+    M2 TN = transfer(np, nq, N, nullptr, nullptr);
+    M2 WL = inv_i_minus(TN);
+    f->Wline[0] = (double)WL.a; f->Wline[1] = (double)WL.b; f->Wline[2] = (double)WL.c; f->Wline[3] = (double)WL.d;
+
+    if (LC == 0) return 0;
+    if (N % LC != 0 || N / LC > CH_MAX_P || LC < 2) return -1;
+    f->LC = LC; f->P = N / LC;
+    ld alpha[CH_MAX_LC], beta[CH_MAX_LC];
+    M2 M = transfer(np, nq, LC, alpha, beta);
+    for (int k = 0; k < LC; ++k) { f->alpha[k] = (double)alpha[k]; f->beta[k] = (double)beta[k]; }
+    // K: neighbours to sum.  Truncate when M^K is far below one ulp of the data, else close exactly.
+    int K = f->P;
+    {
+        M2 pw = { 1, 0, 0, 1 };
+        for (int j = 1; j < f->P; ++j) {
+            pw = mul(pw, M);
+            if (maxabs(pw) < 1e-22L) { K = j; break; }
+        }
+    }
+    f->K = K;
+    M2 close = { 1, 0, 0, 1 };
+    if (K == f->P) {
+        M2 MP = { 1, 0, 0, 1 };
+        for (int j = 0; j < f->P; ++j) MP = mul(MP, M);
+        close = inv_i_minus(MP);
+    }
+    M2 pw = close;
+    for (int j = 0; j < K; ++j) {
+        f->W[j][0] = (double)pw.a; f->W[j][1] = (double)pw.b; f->W[j][2] = (double)pw.c; f->W[j][3] = (double)pw.d;
+        pw = mul(M, pw);
+    }
+    return 0;
+}

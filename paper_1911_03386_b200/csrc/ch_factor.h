@@ -1,0 +1,39 @@
+// ch_factor.h -- host-side periodic (circulant) LU factorisation of
+//   A = I + s (delta^2)^2 = circulant(s, -4s, 1+6s, -4s, s),   s = gamma dt      (include/ch.h)
+//
+// A is a circulant, so its symbol factors exactly (spectral factorisation):
+//   s z^2 - 4 s z + (1+6s) - 4 s z^-1 + s z^-2 = c0 (1 + p z^-1 + q z^-2)(1 + p z + q z^2)
+// with the two roots of 1 + p z^-1 + q z^-2 inside the unit circle.  Replacing z by the
+// cyclic shift gives A = c0 * U * L with L = I + p S^-1 + q S^-2 (cyclic lower band) and
+// U = L^T: the periodic LU factorisation with constant bands.  A v = b is then two cyclic
+// two-term recurrences
+//   forward : z_i = b_i - p z_{i-1} - q z_{i-2}            (indices mod N)
+//   backward: v_i = z_i - p v_{i+1} - q v_{i+2},   result v / c0
+// and each cyclic recurrence is solved chunk-parallel: every chunk of LC points runs from a
+// zero state, the true state entering chunk c is
+//   s_in(c) = sum_{j>=1} M^{j-1} out(c-j)       M = transfer matrix of one chunk,
+// closed over the period by (I - M^P)^-1 (this is the Sherman-Morrison/Woodbury closure of
+// the periodic factorisation), and the chunk is corrected by alpha_k a + beta_k b.
+// Everything below is O(LC + P) doubles per (N, s), shared by all lines, axes and members.
+#pragma once
+
+#define CH_MAX_LC 32      // longest chunk a thread holds in registers
+#define CH_MAX_P 128      // most chunks per line on the chunked path
+
+struct ChFactor {
+    double sigma;
+    double np, nq;             // -p, -q of the recurrence
+    double c0;                 // A = c0 U L
+    double rho;                // modulus of the roots inside the unit circle
+    // chunked path
+    int LC, P, K;              // chunk length, chunks per line, neighbours summed (K == P: closed exactly)
+    double alpha[CH_MAX_LC];   // homogeneous solutions: u_k for (u_-1,u_-2) = (1,0)
+    double beta[CH_MAX_LC];    //                                   ... = (0,1)
+    double W[CH_MAX_P][4];     // W_j = M^{j-1} (I - M^P)^-1 (K == P) or M^{j-1} (K < P), row-major 2x2
+    // generic path (one thread per line): closure of the whole line, (I - T^N)^-1
+    double Wline[4];
+};
+
+// Fill f for line length N and chunk length LC (LC == 0: generic path only).
+// Returns 0, or -1 if the factorisation failed its self-check.
+int ch_factor_build(ChFactor *f, int N, double sigma, int LC);

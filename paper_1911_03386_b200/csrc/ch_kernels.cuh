@@ -1,0 +1,391 @@
+// ch_kernels.cuh -- device kernels of libch (sm_100a, fp64).  See DESIGN.md for the
+// data layout, the per-kernel byte model and the roofline each kernel is bound by.
+//
+//   k_rhs2d / k_rhs3d    r = scale * Lap_h mu(C)   (+ fused F, Fdot, mass partials)   include/ch.h
+//   k_finish             deterministic finish of the partials -> {F, Fdot, beta, mass} P:64
+//   k_sweep_contig       w := A_x^-1 w, lines contiguous (x), chunked periodic LU      ch_factor.h
+//   k_sweep_strided      w := A_d^-1 w, lines at a stride (y, z), optional C += w
+//   k_sweep_generic      any N >= 8: one thread per line, four passes through global memory
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ch_factor.h"
+
+struct SweepParams {
+    double np, nq;              // recurrence  z_i = b_i + np z_{i-1} + nq z_{i-2}
+    double oscale;              // output scale (1/c0 for the stand-alone ch_sweep, unused in the step)
+    double alpha[CH_MAX_LC];
+    double beta[CH_MAX_LC];
+    const double *W;            // device [K][4]
+    int K, P;
+};
+
+// ------------------------------------------------------------------------------------
+// reductions
+// ------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum three values over a block of NW warps in a fixed order; result valid in thread 0.
+template <int NW>
+__device__ __forceinline__ void block_sum3(double &a, double &b, double &c, double (*red)[3])
+{
+    a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { red[wid][0] = a; red[wid][1] = b; red[wid][2] = c; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a = red[0][0]; b = red[0][1]; c = red[0][2];
+#pragma unroll
+        for (int w = 1; w < NW; ++w) { a += red[w][0]; b += red[w][1]; c += red[w][2]; }
+    }
+}
+
+template <bool POW2>
+__device__ __forceinline__ int wrapi(int i, int N)
+{
+    if (POW2) return i & (N - 1);
+    i %= N;
+    return i < 0 ? i + N : i;
+}
+
+// ------------------------------------------------------------------------------------
+// RHS, 2D.  Tile TX x TY per CTA, C staged with halo 2, mu with halo 1 in shared memory.
+// grid = (tiles_x * tiles_y, ensemble), block = 256.
+// ------------------------------------------------------------------------------------
+#define RHS2_TX 64
+#define RHS2_TY 32
+
+template <bool DIAG, bool WRITE, bool POW2>
+__global__ void __launch_bounds__(256) k_rhs2d(const double *__restrict__ C, double *__restrict__ r,
+                                               double *__restrict__ partials, int N, double gamma, double scale,
+                                               int tiles_x)
+{
+    constexpr int TX = RHS2_TX, TY = RHS2_TY, CW = TX + 4, MW = TX + 2;
+    __shared__ double sC[(TY + 4) * CW];
+    __shared__ double sMu[(TY + 2) * MW];
+    __shared__ double red[8][3];
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.x, m = blockIdx.y;
+    const int x0 = (tile % tiles_x) * TX, y0 = (tile / tiles_x) * TY;
+    const double *Cm = C + (size_t)m * N * N;
+
+    for (int i = tid; i < (TY + 4) * CW; i += 256) {
+        const int ly = i / CW, lx = i - ly * CW;
+        const int gy = wrapi<POW2>(y0 + ly - 2, N), gx = wrapi<POW2>(x0 + lx - 2, N);
+        sC[i] = Cm[(size_t)gy * N + gx];
+    }
+    __syncthreads();
+    for (int i = tid; i < (TY + 2) * MW; i += 256) {
+        const int ly = i / MW, lx = i - ly * MW;
+        const double *p = sC + (ly + 1) * CW + lx + 1;
+        const double c = p[0];
+        const double lap = (p[1] + p[-1]) + (p[CW] + p[-CW]) - 4.0 * c;
+        sMu[i] = c * c * c - c - gamma * lap;
+    }
+    __syncthreads();
+    double F = 0.0, Fd = 0.0, ms = 0.0;
+    for (int i = tid; i < TY * TX; i += 256) {
+        const int ly = i / TX, lx = i - ly * TX;
+        const int gy = y0 + ly, gx = x0 + lx;
+        if (gy < N && gx < N) {
+            const double *q = sMu + (ly + 1) * MW + lx + 1;
+            const double mu = q[0];
+            if (WRITE) {
+                const double lap = (q[1] + q[-1]) + (q[MW] + q[-MW]) - 4.0 * mu;
+                r[(size_t)m * N * N + (size_t)gy * N + gx] = scale * lap;
+            }
+            if (DIAG) {
+                const double *p = sC + (ly + 2) * CW + lx + 2;
+                const double c = p[0], dcx = p[1] - c, dcy = p[CW] - c;
+                const double dmx = q[1] - mu, dmy = q[MW] - mu;
+                const double w = c * c - 1.0;
+                F += 0.25 * w * w + 0.5 * gamma * (dcx * dcx + dcy * dcy);
+                Fd -= dmx * dmx + dmy * dmy;
+                ms += c;
+            }
+        }
+    }
+    if (DIAG) {
+        block_sum3<8>(F, Fd, ms, red);
+        if (tid == 0) {
+            double *o = partials + ((size_t)m * gridDim.x + tile) * 3;
+            o[0] = F; o[1] = Fd; o[2] = ms;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// RHS, 3D.  Tile 32 x 8 x 8 per CTA, dynamic shared memory.
+// grid = (tiles_x * tiles_y * tiles_z, ensemble), block = 256.
+// ------------------------------------------------------------------------------------
+#define RHS3_TX 32
+#define RHS3_TY 8
+#define RHS3_TZ 8
+#define RHS3_SMEM (((RHS3_TZ + 4) * (RHS3_TY + 4) * (RHS3_TX + 4) + (RHS3_TZ + 2) * (RHS3_TY + 2) * (RHS3_TX + 2)) * 8)
+
+template <bool DIAG, bool WRITE, bool POW2>
+__global__ void __launch_bounds__(256) k_rhs3d(const double *__restrict__ C, double *__restrict__ r,
+                                               double *__restrict__ partials, int N, double gamma, double scale,
+                                               int tiles_x, int tiles_y)
+{
+    constexpr int TX = RHS3_TX, TY = RHS3_TY, TZ = RHS3_TZ;
+    constexpr int CW = TX + 4, CH = TY + 4, CD = TZ + 4, MW = TX + 2, MH = TY + 2, MD = TZ + 2;
+    extern __shared__ double smem3[];
+    double *sC = smem3, *sMu = smem3 + CD * CH * CW;
+    __shared__ double red[8][3];
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.x, m = blockIdx.y;
+    const int x0 = (tile % tiles_x) * TX, y0 = ((tile / tiles_x) % tiles_y) * TY, z0 = (tile / (tiles_x * tiles_y)) * TZ;
+    const size_t n2 = (size_t)N * N;
+    const double *Cm = C + (size_t)m * n2 * N;
+
+    for (int i = tid; i < CD * CH * CW; i += 256) {
+        const int lz = i / (CH * CW), rem = i - lz * (CH * CW), ly = rem / CW, lx = rem - ly * CW;
+        const int gz = wrapi<POW2>(z0 + lz - 2, N), gy = wrapi<POW2>(y0 + ly - 2, N), gx = wrapi<POW2>(x0 + lx - 2, N);
+        sC[i] = Cm[gz * n2 + (size_t)gy * N + gx];
+    }
+    __syncthreads();
+    for (int i = tid; i < MD * MH * MW; i += 256) {
+        const int lz = i / (MH * MW), rem = i - lz * (MH * MW), ly = rem / MW, lx = rem - ly * MW;
+        const double *p = sC + ((lz + 1) * CH + ly + 1) * CW + lx + 1;
+        const double c = p[0];
+        const double lap = (p[1] + p[-1]) + (p[CW] + p[-CW]) + (p[CH * CW] + p[-CH * CW]) - 6.0 * c;
+        sMu[i] = c * c * c - c - gamma * lap;
+    }
+    __syncthreads();
+    double F = 0.0, Fd = 0.0, ms = 0.0;
+    for (int i = tid; i < TZ * TY * TX; i += 256) {
+        const int lz = i / (TY * TX), rem = i - lz * (TY * TX), ly = rem / TX, lx = rem - ly * TX;
+        const int gz = z0 + lz, gy = y0 + ly, gx = x0 + lx;
+        if (gz < N && gy < N && gx < N) {
+            const double *q = sMu + ((lz + 1) * MH + ly + 1) * MW + lx + 1;
+            const double mu = q[0];
+            if (WRITE) {
+                const double lap = (q[1] + q[-1]) + (q[MW] + q[-MW]) + (q[MH * MW] + q[-MH * MW]) - 6.0 * mu;
+                r[(size_t)m * n2 * N + gz * n2 + (size_t)gy * N + gx] = scale * lap;
+            }
+            if (DIAG) {
+                const double *p = sC + ((lz + 2) * CH + ly + 2) * CW + lx + 2;
+                const double c = p[0], dcx = p[1] - c, dcy = p[CW] - c, dcz = p[CH * CW] - c;
+                const double dmx = q[1] - mu, dmy = q[MW] - mu, dmz = q[MH * MW] - mu;
+                const double w = c * c - 1.0;
+                F += 0.25 * w * w + 0.5 * gamma * (dcx * dcx + dcy * dcy + dcz * dcz);
+                Fd -= dmx * dmx + dmy * dmy + dmz * dmz;
+                ms += c;
+            }
+        }
+    }
+    if (DIAG) {
+        block_sum3<8>(F, Fd, ms, red);
+        if (tid == 0) {
+            double *o = partials + ((size_t)m * gridDim.x + tile) * 3;
+            o[0] = F; o[1] = Fd; o[2] = ms;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// Finish: out[m] = {F, Fdot, beta, mass}, beta = -t Fdot / F (0 if F == 0).
+// grid = ensemble, block = 128; fixed summation order (bitwise reproducible).
+// ------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_finish(const double *__restrict__ partials, int nparts,
+                                                double *__restrict__ out, double t)
+{
+    __shared__ double red[4][3];
+    const int m = blockIdx.x;
+    const double *p = partials + (size_t)m * nparts * 3;
+    double F = 0.0, Fd = 0.0, ms = 0.0;
+    for (int i = threadIdx.x; i < nparts; i += 128) { F += p[3 * i]; Fd += p[3 * i + 1]; ms += p[3 * i + 2]; }
+    block_sum3<4>(F, Fd, ms, red);
+    if (threadIdx.x == 0) {
+        double *o = out + (size_t)m * 4;
+        o[0] = F; o[1] = Fd; o[2] = (F == 0.0) ? 0.0 : -t * Fd / F; o[3] = ms;
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// Chunked periodic-LU line solve on LC points held in registers (see ch_factor.h).
+// Every thread owns chunk `c` of one line; sa/sb are the shared exchange slots of that
+// line, indexed [chunk * cstride].  All threads of the CTA must call this together.
+// ------------------------------------------------------------------------------------
+template <int LC>
+__device__ __forceinline__ void chunk_state_in(const SweepParams &prm, const double *sa, const double *sb,
+                                               int c, int cstride, int dir, double &a, double &b)
+{
+    a = 0.0; b = 0.0;
+    const int P = prm.P;
+    int s = c;
+    for (int j = 0; j < prm.K; ++j) {
+        s -= dir;
+        if (s < 0) s += P;
+        if (s >= P) s -= P;
+        const double oa = sa[s * cstride], ob = sb[s * cstride];
+        const double2 W01 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j);
+        const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
+        a = fma(W01.x, oa, fma(W01.y, ob, a));
+        b = fma(W23.x, oa, fma(W23.y, ob, b));
+    }
+}
+
+template <int LC>
+__device__ __forceinline__ void chunk_solve(const SweepParams &prm, double (&v)[LC], double *sa, double *sb,
+                                            int c, int cstride)
+{
+    const double np = prm.np, nq = prm.nq;
+    double a, b;
+    // forward: z_k = b_k + np z_{k-1} + nq z_{k-2}, zero state
+    v[1] = fma(np, v[0], v[1]);
+#pragma unroll
+    for (int k = 2; k < LC; ++k) v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k]));
+    sa[c * cstride] = v[LC - 1];
+    sb[c * cstride] = v[LC - 2];
+    __syncthreads();
+    chunk_state_in<LC>(prm, sa, sb, c, cstride, +1, a, b);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
+    __syncthreads();
+    // backward: x_k = z_k + np x_{k+1} + nq x_{k+2}, zero state
+    v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
+#pragma unroll
+    for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
+    sa[c * cstride] = v[0];
+    sb[c * cstride] = v[1];
+    __syncthreads();
+    chunk_state_in<LC>(prm, sa, sb, c, cstride, -1, a, b);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
+}
+
+// ------------------------------------------------------------------------------------
+// Strided sweep (y, z): thread (tx, c) owns chunk c of the line through inner position tx.
+// block = (COLS, P); grid.x = inner_blocks * n_outer.  A warp reads COLS*8 contiguous bytes
+// per line point.  UPDATE: C += w instead of writing w (last sweep of the step).
+// ------------------------------------------------------------------------------------
+template <int LC, bool UPDATE, bool SCALE>
+__global__ void __launch_bounds__(512) k_sweep_strided(const __grid_constant__ SweepParams prm, double *__restrict__ w,
+                                double *__restrict__ C, size_t outer_stride, size_t line_stride, int inner_blocks)
+{
+    extern __shared__ double sx[];
+    const int COLS = blockDim.x, P = blockDim.y;
+    const int tx = threadIdx.x, c = threadIdx.y;
+    const int ib = blockIdx.x % inner_blocks, o = blockIdx.x / inner_blocks;
+    const size_t base = (size_t)o * outer_stride + (size_t)c * LC * line_stride + (size_t)ib * COLS + tx;
+    double *sa = sx + tx, *sb = sx + P * COLS + tx;
+
+    double v[LC];
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = w[base + k * line_stride];
+    chunk_solve<LC>(prm, v, sa, sb, c, COLS);
+    if (UPDATE) {
+#pragma unroll
+        for (int k0 = 0; k0 < LC; k0 += 8) {
+            double cc[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) cc[k] = C[base + (k0 + k) * line_stride];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) C[base + (k0 + k) * line_stride] = cc[k] + v[k0 + k];
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < LC; ++k) w[base + k * line_stride] = SCALE ? v[k] * prm.oscale : v[k];
+    }
+}
+
+// ------------------------------------------------------------------------------------
+// Contiguous sweep (x): CTA = LPB consecutive lines, thread (l, c) = chunk c of line l.
+// Lines are staged through shared memory with a 16-byte-granule XOR swizzle so that both
+// the coalesced global phase and the chunk phase (LDS.128, lane stride LC*8 bytes) are
+// bank-conflict free.  block = LPB * P threads, dynamic smem = LPB*N*8 + 2*LPB*P*8.
+// ------------------------------------------------------------------------------------
+template <int LC>
+__device__ __forceinline__ int swz(int g)
+{
+    constexpr int SH = LC == 8 ? 2 : (LC == 16 ? 3 : 4);
+    return g ^ ((g >> SH) & 7);
+}
+
+template <int LC, bool SCALE>
+__global__ void k_sweep_contig(const __grid_constant__ SweepParams prm, double *__restrict__ w, int N,
+                               long long total_lines, int LPB)
+{
+    extern __shared__ double2 sl[];
+    const int P = prm.P;
+    const int nthreads = blockDim.x, t = threadIdx.x;
+    const long long line0 = (long long)blockIdx.x * LPB;
+    const int nlines = (int)((total_lines - line0) < LPB ? (total_lines - line0) : LPB);
+    const int G = nlines * (N / 2);                           // granules held by this CTA
+    double2 *g2 = reinterpret_cast<double2 *>(w + (size_t)line0 * N);
+    double *sa = reinterpret_cast<double *>(sl + (size_t)LPB * (N / 2));
+    double *sb = sa + LPB * P;
+
+    for (int g = t; g < G; g += nthreads) sl[swz<LC>(g)] = g2[g];
+    __syncthreads();
+
+    const int l = t / P, c = t - l * P;
+    const int gbase = l * (N / 2) + c * (LC / 2);
+    double v[LC];
+    const bool live = l < nlines;
+#pragma unroll
+    for (int k = 0; k < LC / 2; ++k) {
+        double2 x = live ? sl[swz<LC>(gbase + k)] : make_double2(0.0, 0.0);
+        v[2 * k] = x.x; v[2 * k + 1] = x.y;
+    }
+    chunk_solve<LC>(prm, v, sa + l * P, sb + l * P, c, 1);
+    if (live) {
+#pragma unroll
+        for (int k = 0; k < LC / 2; ++k) {
+            double2 x;
+            x.x = SCALE ? v[2 * k] * prm.oscale : v[2 * k];
+            x.y = SCALE ? v[2 * k + 1] * prm.oscale : v[2 * k + 1];
+            sl[swz<LC>(gbase + k)] = x;
+        }
+    }
+    __syncthreads();
+    for (int g = t; g < G; g += nthreads) g2[g] = sl[swz<LC>(g)];
+}
+
+// ------------------------------------------------------------------------------------
+// Generic sweep, any N >= 8: one thread per line, the cyclic recurrences run through
+// global memory (four passes).  Correct for every N; slow.  lines are enumerated as
+// (outer, inner): address = outer * outer_stride + inner * inner_stride + i * line_stride.
+// ------------------------------------------------------------------------------------
+template <bool UPDATE>
+__global__ void __launch_bounds__(128) k_sweep_generic(double np, double nq, double W0, double W1, double W2, double W3,
+                                                       double oscale, double *__restrict__ w, double *__restrict__ C,
+                                                       int N, long long n_lines, int n_inner, size_t outer_stride,
+                                                       size_t inner_stride, size_t line_stride)
+{
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= n_lines) return;
+    const size_t base = (size_t)(id / n_inner) * outer_stride + (size_t)(id % n_inner) * inner_stride;
+    double *x = w + base;
+    double z1 = 0.0, z2 = 0.0;
+    for (int i = 0; i < N; ++i) {
+        const double z = fma(np, z1, fma(nq, z2, x[i * line_stride]));
+        x[i * line_stride] = z; z2 = z1; z1 = z;
+    }
+    double u1 = W0 * z1 + W1 * z2, u2 = W2 * z1 + W3 * z2;
+    for (int i = 0; i < N; ++i) {
+        const double u = np * u1 + nq * u2;
+        x[i * line_stride] += u; u2 = u1; u1 = u;
+    }
+    z1 = 0.0; z2 = 0.0;
+    for (int i = N - 1; i >= 0; --i) {
+        const double z = fma(np, z1, fma(nq, z2, x[i * line_stride]));
+        x[i * line_stride] = z; z2 = z1; z1 = z;
+    }
+    u1 = W0 * z1 + W1 * z2; u2 = W2 * z1 + W3 * z2;
+    for (int i = N - 1; i >= 0; --i) {
+        const double u = np * u1 + nq * u2;
+        const double val = (x[i * line_stride] + u) * oscale;
+        if (UPDATE) C[base + i * line_stride] += val; else x[i * line_stride] = val;
+        u2 = u1; u1 = u;
+    }
+}
