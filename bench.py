@@ -1,0 +1,289 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ensemble Cahn-Hilliard ADI step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+
+A "step" is one time step of the whole hot path (RHS stencil -> one cyclic-pentadiagonal sweep
+per axis -> fused update, with the F/dF/dt/mass reduction at the config's sampling stride) over
+the whole ensemble of the workload.  metric = grid-point updates per second.  One JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1911_03386_b200 import inputs  # noqa: E402
+
+METRIC = "grid-point updates/sec (fp64 ensemble CH ADI step)"
+UNIT = "updates/s"
+FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+# Algorithmic bytes per grid-point update per kernel:
+# every kernel reads and writes one fp64 field; the last sweep also reads C^n for the fused update.
+ALGO_BYTES = {
+    2: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 24},
+    3: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 16, "sweep_z": 24},
+}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/), keyed by (workload, kernel); None until captured.
+NCU_TRAFFIC_BYTES = {}
+
+
+def workload_desc(name):
+    c = inputs.CONFIGS[name]
+    return f"{name}: {c['D']}D {'x'.join([str(c['N'])] * c['D'])} x {c['ensemble']} members, gamma={c['gamma']}, dt={c['dt']}, stride={c['stride']}"
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    FIELDS = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- oracle legs
+def oracle_sample(name, steps, warmup=0, max_members=None):
+    """Time the CPU oracle, as it stands, on a bounded sample of the workload: the first
+    min(cores, ensemble) members (OpenMP over members), `steps` time steps."""
+    from oracle import ch_oracle
+    c = inputs.CONFIGS[name]
+    cores = ch_oracle.num_threads()
+    members = min(cores, c["ensemble"]) if max_members is None else min(max_members, c["ensemble"])
+    C0 = inputs.config_state(name, members=range(members))
+    if warmup:
+        C0 = ch_oracle.step(C0, c["gamma"], c["dt"], warmup)
+    t = time.perf_counter()
+    ch_oracle.step(C0, c["gamma"], c["dt"], steps)
+    dt = time.perf_counter() - t
+    updates = members * c["N"] ** c["D"] * steps
+    return {"value": updates / dt, "unit": UNIT, "cores": min(cores, members), "kind": "oracle",
+            "sample": f"first {members} of {c['ensemble']} members of {name}, {steps} steps, gcc -O2 -fopenmp over members",
+            "seconds": dt, "ms_per_step": dt / steps * 1e3}
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    name = args.workload
+    c = inputs.CONFIGS[name]
+    r = oracle_sample(name, args.steps, warmup=args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_desc(name), "note": "CPU oracle on host cores; each step is one time step of a bounded member sample"},
+        "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------- CUDA arm
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def run_ours(args):
+    import torch
+    from paper_1911_03386_b200 import binding as B, build
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path is the only path (no CPU fallback)")
+    build.build()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1911_03386_b200 import shard
+
+    name = args.workload
+    c = inputs.CONFIGS[name]
+    M, N, D, stride = c["ensemble"], c["N"], c["D"], c["stride"]
+    pts = M * N ** D
+    K, W = args.steps, args.warmup
+
+    # weak scaling: every rank steps its own full ensemble (disjoint seeds), no data-path collective
+    seeds_off = rank * M
+    cb = c["cbar"]
+    cbars = cb if isinstance(cb, (list, tuple)) else [cb] * M
+    host = torch.empty((M,) + (N,) * D, dtype=torch.float64).pin_memory()
+    host.numpy()[...] = inputs.initial_state([c["seed0"] + seeds_off + k for k in range(M)], N, D, cbars, c["amp"])
+    host_out = torch.empty_like(host).pin_memory()
+
+    stream = torch.cuda.current_stream()
+    ens = B.Ensemble(M, N, D, c["gamma"], c["dt"], stream=stream.cuda_stream)
+    cap = (W + K) // stride + 2
+    dstate = host.to(dev, non_blocking=True)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident leg: inputs already in HBM when the timed region starts
+    ens.set_state(dstate)
+    ens.set_series(stride, cap)
+    ens.step(W)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    l0 = B.ch_launch_count(ens.ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    ens.step(K)
+    e1.record(stream)
+    barrier()
+    launches = B.ch_launch_count(ens.ctx) - l0
+    secs = shard.max_over_ranks(e0.elapsed_time(e1) * 1e-3, device=dev)
+    time.sleep(0.15)
+    clocks = sampler.stop()
+    value = world * pts * K / secs
+
+    # ---- per-kernel leg: same steps with every launch bracketed by CUDA events on the stream
+    B.ch_profile(ens.ctx, 1)
+    ens.set_state(dstate)
+    ens.set_series(stride, cap)
+    ens.step(W)
+    B.ch_profile_read(ens.ctx)
+    ens.step(K)
+    prof = B.ch_profile_read(ens.ctx)
+    B.ch_profile(ens.ctx, 0)
+    peak, peak_src = measured_peak()
+    kernels = {}
+    for kind, (ms, cnt) in prof.items():
+        if cnt and kind in ALGO_BYTES[D]:
+            avg = ms / cnt
+            gbs = pts * ALGO_BYTES[D][kind] / (avg * 1e-3) / 1e9
+            kernels[kind] = {"launches": cnt, "avg_ms": avg, "algo_bytes_per_update": ALGO_BYTES[D][kind],
+                             "achieved_gbs": gbs, "frac": gbs / peak}
+    total_kernel_ms = sum(ms for ms, _ in prof.values())
+    main_kinds = {k: v for k, v in kernels.items() if k != "rhs_diag"} or kernels
+    dom = max(main_kinds, key=lambda k: main_kinds[k]["avg_ms"] * main_kinds[k]["launches"])
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES.get((name, dom)),
+                "peak_source": peak_src, "share_of_step": kernels[dom]["avg_ms"] * kernels[dom]["launches"] / total_kernel_ms,
+                "step_algo_bytes_per_update": 56 if D == 2 else 72,
+                "step_achieved_gbs": value / world * (56 if D == 2 else 72) / 1e9,
+                "step_frac": value / world * (56 if D == 2 else 72) / 1e9 / peak,
+                "step_frac_of_8TBs_nominal": value / world * (56 if D == 2 else 72) / 1e9 / 8000.0}
+
+    # ---- end-to-end leg: the user's job through the C ABI with HOST buffers (pinned):
+    # ch_set_state(host) -> ch_step(K) with the series -> series D2H + ch_energy(host) + ch_get_state(host)
+    series_host = torch.empty((cap, M, 4), dtype=torch.float64).pin_memory()
+    eout = np.empty((M, 4), dtype=np.float64)
+    barrier()
+    t0 = time.perf_counter()
+    B.ch_set_state(ens.ctx, host.numpy())
+    ens.set_series(stride, cap)
+    ens.step(K)
+    B.ch_energy(ens.ctx, eout)
+    B.ch_get_state(ens.ctx, host_out.numpy())
+    ns = B.ch_series_count(ens.ctx)
+    series_host[:ns].copy_(ens._series[:ns], non_blocking=True)
+    barrier()
+    e2e_secs = shard.max_over_ranks(time.perf_counter() - t0, device=dev)
+    state_bytes = pts * 8
+    e2e = {"value": world * pts * K / e2e_secs, "unit": UNIT,
+           "h2d_bytes_per_step": state_bytes / K, "d2h_bytes_per_step": (state_bytes + ns * M * 32 + M * 32) / K,
+           "seconds": e2e_secs, "job": f"ch_set_state(host {state_bytes >> 20} MiB) + ch_step({K}) + series/energy/state to host"}
+    assert np.isfinite(eout).all() and np.isfinite(host_out.numpy()).all()
+
+    ens.close()
+    if rank == 0:
+        cpu = oracle_sample(name, max(5, int(1.5e8 / N ** D)))    # ~10-20 s of CPU work per core
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": secs / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_desc(name), "members_per_gpu": M, "parallelism": f"ensemble-sharded x{world} (no data-path collective)",
+                       "l2": f"working set {2 * state_bytes >> 20} MiB per GPU, larger than the 126 MB L2; no explicit flush",
+                       "sampling": f"F, dF/dt, beta, mass every {stride} steps inside the timed region"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline, "kernels": kernels,
+            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        }
+        print(json.dumps(line))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--workload", default="cfg3", choices=sorted(inputs.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

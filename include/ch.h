@@ -121,14 +121,21 @@ long long ch_step_count(const ch_ctx *ctx);
 int ch_rhs(ch_ctx *ctx, double *r_out, int on_device);
 int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
 
-/* Kernel-variant and launch options (measurement knobs; every variant computes the same step):
- *   "graph"      0/1   replay one sampling period as a CUDA graph (default 1)
- *   "sweep"      0     auto, 1 force the generic thread-per-line sweeps, 2 force the chunked sweeps
- *   "fuse_rhs_x" 0/1   fuse the RHS stencil into the x-sweep kernel where supported (default 1)
- *   "batch"      k     advance k members at a time through a whole sampling period so that
- *                      their state stays L2-resident (0 = whole ensemble per launch)          */
+/* Kernel-variant options (measurement knobs; every variant computes the same step):
+ *   "sweep"   0 auto, 1 force the generic thread-per-line sweeps, 2 force the chunked sweeps
+ * ch_get_option also answers "chunked" (chunk length of the fast sweeps, 0 if N needs the
+ * generic path) and "K" (chunk neighbours summed by the periodic closure). */
 int ch_set_option(ch_ctx *ctx, const char *key, int value);
 int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
+
+/* Per-kernel device timing.  ch_profile(ctx, 1) makes every later launch be bracketed by CUDA
+ * events on the context's stream; ch_profile_read synchronises, returns the summed milliseconds
+ * and launch counts per kernel kind (ch_kernel_kinds() kinds, named by ch_kernel_kind_name:
+ * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z) and clears the records. */
+int ch_profile(ch_ctx *ctx, int enable);
+int ch_profile_read(ch_ctx *ctx, double *ms, long long *counts, int nkinds);
+int ch_kernel_kinds(void);
+const char *ch_kernel_kind_name(int kind);
 
 /* Kernel launches enqueued by this context since creation (each graph node counts once per replay). */
 long long ch_launch_count(const ch_ctx *ctx);

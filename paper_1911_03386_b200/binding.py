@@ -19,7 +19,8 @@ EXPORTS = [
     "ch_create", "ch_destroy", "ch_set_stream", "ch_workspace_bytes", "ch_attach_workspace",
     "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_energy", "ch_get_state",
     "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
-    "ch_launch_count", "ch_last_error",
+    "ch_launch_count", "ch_last_error", "ch_profile", "ch_profile_read", "ch_kernel_kinds",
+    "ch_kernel_kind_name",
 ]
 
 _LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libch.so")
@@ -62,6 +63,11 @@ def lib():
         L.ch_get_option.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ci)]
         L.ch_launch_count.argtypes = [vp]
         L.ch_launch_count.restype = ctypes.c_longlong
+        L.ch_profile.argtypes = [vp, ci]
+        L.ch_profile_read.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong), ci]
+        L.ch_kernel_kinds.restype = ci
+        L.ch_kernel_kind_name.argtypes = [ci]
+        L.ch_kernel_kind_name.restype = ctypes.c_char_p
         L.ch_last_error.argtypes = [vp]
         L.ch_last_error.restype = ctypes.c_char_p
         _lib = L
@@ -167,6 +173,19 @@ def ch_get_option(ctx, key):
 
 def ch_launch_count(ctx):
     return lib().ch_launch_count(ctx)
+
+
+def ch_profile(ctx, enable):
+    _check(ctx, lib().ch_profile(ctx, int(enable)))
+
+
+def ch_profile_read(ctx):
+    """{kind name: (total ms, launches)} since profiling was switched on / last read."""
+    n = lib().ch_kernel_kinds()
+    ms = (ctypes.c_double * n)()
+    cnt = (ctypes.c_longlong * n)()
+    _check(ctx, lib().ch_profile_read(ctx, ms, cnt, n))
+    return {lib().ch_kernel_kind_name(k).decode(): (ms[k], cnt[k]) for k in range(n)}
 
 
 # ---- convenience wrapper ---------------------------------------------------------------

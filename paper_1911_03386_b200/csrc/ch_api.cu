@@ -5,10 +5,16 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/ch.h"
 #include "ch_factor.h"
 #include "ch_kernels.cuh"
+
+enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z, KIND_COUNT };
+static const char *const kKindNames[KIND_COUNT] = { "rhs", "rhs_diag", "finish", "sweep_x", "sweep_y", "sweep_z" };
+
+struct ProfRec { int kind; cudaEvent_t e0, e1; };
 
 struct ch_ctx {
     int M, N, D;
@@ -40,7 +46,27 @@ struct ch_ctx {
     // options
     int opt_sweep;          // 0 auto, 1 generic, 2 chunked
     long long launches;
+    bool profiling;
+    std::vector<ProfRec> prof;
     std::string err;
+};
+
+// Brackets one kernel launch with CUDA events on the context's stream when profiling is on.
+struct ProfScope {
+    ch_ctx *c; int kind; cudaEvent_t e0;
+    ProfScope(ch_ctx *ctx, int k) : c(ctx), kind(k), e0(nullptr)
+    {
+        if (c->profiling && cudaEventCreate(&e0) == cudaSuccess) cudaEventRecord(e0, c->stream);
+    }
+    ~ProfScope()
+    {
+        c->launches++;
+        if (!e0) return;
+        cudaEvent_t e1;
+        if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return; }
+        cudaEventRecord(e1, c->stream);
+        c->prof.push_back({ kind, e0, e1 });
+    }
 };
 
 static thread_local std::string g_create_err;
@@ -126,7 +152,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->C = c->w = c->partials = c->eout = nullptr;
     c->has_state = false; c->n = 0; c->t0 = 0.0;
     c->series = nullptr; c->stride = 0; c->capacity = 0; c->cursor = 0; c->last_sampled = -1;
-    c->stream = 0; c->opt_sweep = 0; c->launches = 0;
+    c->stream = 0; c->opt_sweep = 0; c->launches = 0; c->profiling = false;
     if (c->chunked) {
         cudaError_t e = cudaMalloc((void **)&c->dW, sizeof(double) * 4 * CH_MAX_P);
         if (e == cudaSuccess) e = cudaMemcpy(c->dW, c->fac.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
@@ -153,10 +179,17 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     return CH_OK;
 }
 
+static void prof_clear(ch_ctx *ctx)
+{
+    for (auto &r : ctx->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    ctx->prof.clear();
+}
+
 extern "C" int ch_destroy(ch_ctx *ctx)
 {
     if (!ctx) return CH_EINVAL;
     cudaStreamSynchronize(ctx->stream);
+    prof_clear(ctx);
     if (ctx->ws_owned && ctx->ws_base) cudaFree(ctx->ws_base);
     if (ctx->dW) cudaFree(ctx->dW);
     delete ctx;
@@ -232,6 +265,30 @@ extern "C" int ch_series_count(const ch_ctx *ctx) { return ctx ? ctx->cursor : C
 extern "C" long long ch_step_count(const ch_ctx *ctx) { return ctx ? ctx->n : CH_EINVAL; }
 extern "C" long long ch_launch_count(const ch_ctx *ctx) { return ctx ? ctx->launches : CH_EINVAL; }
 
+extern "C" int ch_profile(ch_ctx *ctx, int enable)
+{
+    if (!ctx) return CH_EINVAL;
+    prof_clear(ctx);
+    ctx->profiling = enable != 0;
+    return CH_OK;
+}
+
+extern "C" int ch_profile_read(ch_ctx *ctx, double *ms, long long *counts, int nkinds)
+{
+    if (!ctx || !ms || !counts || nkinds < 1) return CH_EINVAL;
+    for (int k = 0; k < nkinds; ++k) { ms[k] = 0.0; counts[k] = 0; }
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    for (auto &r : ctx->prof) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, r.e0, r.e1) == cudaSuccess && r.kind < nkinds) { ms[r.kind] += t; counts[r.kind]++; }
+    }
+    prof_clear(ctx);
+    return CH_OK;
+}
+
+extern "C" int ch_kernel_kinds(void) { return KIND_COUNT; }
+extern "C" const char *ch_kernel_kind_name(int kind) { return kind >= 0 && kind < KIND_COUNT ? kKindNames[kind] : ""; }
+
 extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
 {
     if (!ctx || !key) return CH_EINVAL;
@@ -259,6 +316,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
 template <bool DIAG, bool WRITE>
 static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
 {
+    ProfScope ps(c, DIAG ? KIND_RHS_DIAG : KIND_RHS);
     if (c->D == 2) {
         dim3 grid(c->nparts, c->M);
         if (c->pow2) k_rhs2d<DIAG, WRITE, true><<<grid, 256, 0, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x);
@@ -268,7 +326,6 @@ static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
         if (c->pow2) k_rhs3d<DIAG, WRITE, true><<<grid, 256, RHS3_SMEM, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x, c->rhs_tiles_y);
         else k_rhs3d<DIAG, WRITE, false><<<grid, 256, RHS3_SMEM, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x, c->rhs_tiles_y);
     }
-    c->launches++;
 }
 
 static void launch_rhs(ch_ctx *c, const double *C, double *r, double scale, bool diag, bool write)
@@ -280,8 +337,8 @@ static void launch_rhs(ch_ctx *c, const double *C, double *r, double scale, bool
 
 static void launch_finish(ch_ctx *c, double *out, double t)
 {
+    ProfScope ps(c, KIND_FINISH);
     k_finish<<<c->M, 128, 0, c->stream>>>(c->partials, c->nparts, out, t);
-    c->launches++;
 }
 
 static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
@@ -298,6 +355,7 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
     const int N = c->N, D = c->D, M = c->M;
     const size_t n2 = (size_t)N * N, n3 = n2 * N;
     const bool chunked = c->chunked && c->opt_sweep != 1;
+    ProfScope ps(c, KIND_SWEEP_X + axis);
     if (!chunked) {
         long long n_lines = (long long)M * (D == 3 ? n2 : (size_t)N);
         int n_inner; size_t os, is, ls;
@@ -308,7 +366,6 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
         const double *Wl = c->fac.Wline;
         if (update) k_sweep_generic<true><<<blocks, 128, 0, c->stream>>>(c->fac.np, c->fac.nq, Wl[0], Wl[1], Wl[2], Wl[3], scale ? oscale : 1.0, w, c->C, N, n_lines, n_inner, os, is, ls);
         else k_sweep_generic<false><<<blocks, 128, 0, c->stream>>>(c->fac.np, c->fac.nq, Wl[0], Wl[1], Wl[2], Wl[3], scale ? oscale : 1.0, w, c->C, N, n_lines, n_inner, os, is, ls);
-        c->launches++;
         return;
     }
     SweepParams prm;
@@ -330,7 +387,6 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
             if (scale) k_sweep_contig<32, true><<<blocks, threads, smem, c->stream>>>(prm, w, N, total_lines, LPB);
             else k_sweep_contig<32, false><<<blocks, threads, smem, c->stream>>>(prm, w, N, total_lines, LPB);
         }
-        c->launches++;
         return;
     }
     // strided
@@ -351,7 +407,6 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
     } while (0)
     if (LC == 16) LAUNCH_STRIDED(16); else LAUNCH_STRIDED(32);
 #undef LAUNCH_STRIDED
-    c->launches++;
 }
 
 static int check_launch(ch_ctx *ctx, const char *what)

@@ -1,0 +1,316 @@
+"""GPU-vs-oracle parity through the C ABI (the parity tests proper).
+
+Tolerances (BASELINE.json north_star): max-abs field difference <= 1e-10 after 1000
+steps; relative error <= 1e-9 on F(t) (and dF/dt, mass), beta compared with relative
+1e-9 plus absolute 1e-12 (beta(0) = 0).  Same seeded inputs on both sides.
+"""
+import numpy as np
+import pytest
+
+from paper_1911_03386_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FIELD_TOL = 1e-10
+SERIES_RTOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1911_03386_b200 import binding, build
+    build.build()
+    return binding
+
+
+def assert_series_close(s, so, rtol=SERIES_RTOL):
+    assert s.shape == so.shape
+    for q in (0, 1, 3):      # F, dF/dt, mass
+        scale = np.maximum(np.abs(so[..., q]), 1e-300)
+        # mass of a symmetric mixture is ~0: compare against sum|C| ~ its natural scale
+        if q == 3:
+            scale = np.maximum(scale, 1.0)
+        assert (np.abs(s[..., q] - so[..., q]) / scale).max() <= rtol, f"series column {q}"
+    assert (np.abs(s[..., 2] - so[..., 2]) <= rtol * np.abs(so[..., 2]) + 1e-12).all(), "beta"
+
+
+def run_gpu(B, C0, gamma, dt, nsteps, stride, options=None, t0=0.0):
+    M, N, D = C0.shape[0], C0.shape[1], C0.ndim - 1
+    e = B.Ensemble(M, N, D, gamma, dt, options=options)
+    e.set_state(C0)
+    if t0:
+        B.ch_set_time(e.ctx, t0)
+    e.set_series(stride, nsteps // stride + 1)
+    e.step(nsteps)
+    C, s = e.get_state(), e.series()
+    e.close()
+    return C, s
+
+
+# ------------------------------------------------------------------ per kernel
+@pytest.mark.parametrize("N,D,M,gamma,dt", [
+    (64, 2, 3, 1.0, 0.01), (512, 2, 2, 1.0, 0.01), (24, 2, 2, 1.0, 0.01), (8, 2, 1, 1.0, 0.01),
+    (100, 2, 1, 0.5, 0.02), (32, 3, 2, 1.0, 0.01), (128, 3, 1, 1.0, 0.01), (20, 3, 1, 1.0, 0.01), (8, 3, 1, 2.0, 0.01),
+])
+def test_rhs_kernel(B, oracle, N, D, M, gamma, dt):
+    C0 = inputs.initial_state(range(50, 50 + M), N, D, -0.2, 0.5)
+    e = B.Ensemble(M, N, D, gamma, dt)
+    e.set_state(C0)
+    r, ro = e.rhs(), oracle.rhs(C0, gamma, dt)
+    e.close()
+    assert np.abs(r - ro).max() <= 1e-13 * np.abs(ro).max()
+
+
+@pytest.mark.parametrize("N,D,M", [(16, 2, 2), (64, 2, 3), (256, 2, 2), (512, 2, 2), (1024, 2, 1), (2048, 2, 1),
+                                   (24, 2, 2), (8, 2, 1), (100, 2, 1), (32, 3, 2), (128, 3, 1), (20, 3, 1)])
+@pytest.mark.parametrize("sigma", [0.01, 1.0, 529.0])
+def test_sweep_kernels(B, oracle, N, D, M, sigma):
+    """Each axis, chunked (N % 16 == 0) or generic path, against the oracle's banded solve.
+    sigma = 529 is the paper's regime (gamma = 0.01, dx = 2 pi/512, dt = 0.0012)."""
+    rng = np.random.default_rng(N * 10 + D)
+    w = rng.standard_normal((M,) + (N,) * D)
+    e = B.Ensemble(M, N, D, sigma / 0.5, 0.5)
+    tol = 1e-14 * (1 + 16 * sigma)
+    for axis in range(D):
+        got, ref = e.sweep(w, axis), oracle.sweep(w, sigma, axis)
+        assert np.abs(got - ref).max() <= tol * np.abs(ref).max(), f"axis {axis}"
+    if B.ch_get_option(e.ctx, "chunked"):
+        B.ch_set_option(e.ctx, "sweep", 1)             # generic kernels on the same data
+        for axis in range(D):
+            got, ref = e.sweep(w, axis), oracle.sweep(w, sigma, axis)
+            assert np.abs(got - ref).max() <= tol * np.abs(ref).max(), f"generic axis {axis}"
+    e.close()
+
+
+def test_energy_kernel(B, oracle):
+    for N, D in [(64, 2), (512, 2), (24, 2), (32, 3), (20, 3)]:
+        C0 = inputs.initial_state([1, 2], N, D, [0.0, -0.4], 0.3)
+        e = B.Ensemble(2, N, D, 1.3, 0.01)
+        e.set_state(C0)
+        got, ref = e.energy(), oracle.energy(C0, 1.3, 0.0)
+        e.close()
+        assert_series_close(got[None], ref[None], 1e-12)
+
+
+# ---------------------------------------------------------------- end to end
+def test_cfg1_full_parity(B, oracle):
+    """configs[0]: 1 member 64^2, every sample of the first 1000 steps and the final field."""
+    c = inputs.CONFIGS["cfg1"]
+    C0 = inputs.config_state("cfg1")
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 1000, c["stride"])
+    Co, so = oracle.run(C0, c["gamma"], c["dt"], 1000, c["stride"])
+    assert s.shape == (101, 1, 4)
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+
+
+def test_cfg1_whole_run(B, oracle):
+    """configs[0] in full: 5000 steps, 501 samples."""
+    c = inputs.CONFIGS["cfg1"]
+    C0 = inputs.config_state("cfg1")
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], c["nsteps"], c["stride"])
+    Co, so = oracle.run(C0, c["gamma"], c["dt"], c["nsteps"], c["stride"])
+    assert s.shape == (501, 1, 4)
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+
+
+def test_cfg2_all_members_short_and_subset_long(B, oracle):
+    c = inputs.CONFIGS["cfg2"]
+    C0 = inputs.config_state("cfg2")
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 1000, c["stride"])
+    sub = [0, 31, 63]
+    Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 1000, c["stride"])
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
+    # all 64 members over 100 steps
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 100, c["stride"])
+    Co, so = oracle.run(C0, c["gamma"], c["dt"], 100, c["stride"])
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+
+
+def test_cfg3_headline_config_member_subset(B, oracle):
+    """configs[2] at full size (128 x 512^2, the shape bench.py times), 1000 steps;
+    members are independent, so the oracle checks the first, the last and one in the middle."""
+    c = inputs.CONFIGS["cfg3"]
+    C0 = inputs.config_state("cfg3")
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 1000, c["stride"])
+    sub = [0, 77, 127]
+    Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 1000, c["stride"])
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
+    # properties at full size: mass conserved, F decreasing, for every member
+    mass, F = s[:, :, 3], s[:, :, 0]
+    assert np.abs(mass - mass[0]).max() <= 1e-9 * np.abs(mass[0]).max()
+    assert (np.diff(F, axis=0) < 0).all()
+
+
+def test_cfg4_3d_member_subset(B, oracle):
+    """configs[3] at full size (16 x 128^3); the oracle follows one member of each mixture for 100 steps."""
+    c = inputs.CONFIGS["cfg4"]
+    C0 = inputs.config_state("cfg4")
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 100, c["stride"])
+    sub = [0, 15]
+    Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 100, c["stride"])
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
+
+
+def test_small_3d_1000_steps(B, oracle):
+    C0 = inputs.initial_state([3000, 3008], 32, 3, [0.0, -0.4], 0.05)
+    C, s = run_gpu(B, C0, 1.0, 0.01, 1000, 50)
+    Co, so = oracle.run(C0, 1.0, 0.01, 1000, 50)
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+
+
+def test_cfg5_long_lines_one_member(B, oracle):
+    """configs[4] at full size (8 x 2048^2); the oracle follows one member for 50 steps."""
+    c = inputs.CONFIGS["cfg5"]
+    C0 = inputs.config_state("cfg5")
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 50, c["stride"])
+    Co, so = oracle.run(C0[[5]], c["gamma"], c["dt"], 50, c["stride"])
+    assert np.abs(C[[5]] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, [5]], so)
+
+
+def test_restart_parity_from_developed_state(B, oracle):
+    """cbar = -0.4 is still linear at step 1000, so also compare from a coarsening state:
+    GPU runs 10000 steps, the state is handed to both sides, compared after 1000 more."""
+    C0 = inputs.initial_state([1000, 2000], 128, 2, [0.0, -0.4], 0.05)
+    e = B.Ensemble(2, 128, 2, 1.0, 0.01)
+    e.set_state(C0)
+    e.step(10000)
+    Cdev = e.get_state()
+    assert np.abs(Cdev).max() > 0.9                       # phase separated
+    e.set_state(Cdev)
+    B.ch_set_time(e.ctx, 100.0)
+    e.set_series(50, 21)
+    e.step(1000)
+    C, s = e.get_state(), e.series()
+    e.close()
+    Co, so = oracle.run(Cdev, 1.0, 0.01, 1000, 50, t0=100.0)
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+    assert (s[:, :, 2] > 0.01).all()                      # beta is O(0.1) here, not ~0
+
+
+def test_paper_regime_large_sigma(B, oracle):
+    """sigma = gamma dt = 529 (the paper's gamma = 0.01, dx = 2 pi/512, dt = 0.0012 in h = 1 units):
+    correction tables do not decay, cond(A) = 8.5e3 per factor."""
+    C0 = inputs.initial_state([7, 8], 128, 2, [0.0, -0.4], 0.05)
+    C, s = run_gpu(B, C0, 66.4, 7.97, 200, 10)
+    Co, so = oracle.run(C0, 66.4, 7.97, 200, 10)
+    assert np.abs(C - Co).max() <= 1e-9
+    assert_series_close(s, so, 1e-7)
+
+
+def test_generic_paths_end_to_end(B, oracle):
+    for N, D, opts in [(24, 2, None), (64, 2, {"sweep": 1}), (8, 2, None), (12, 3, None), (16, 3, {"sweep": 1})]:
+        C0 = inputs.initial_state([11, 12], N, D, [0.0, -0.3], 0.1)
+        C, s = run_gpu(B, C0, 1.0, 0.01, 300, 10, options=opts)
+        Co, so = oracle.run(C0, 1.0, 0.01, 300, 10)
+        assert np.abs(C - Co).max() <= FIELD_TOL, (N, D)
+        assert_series_close(s, so)
+
+
+# ---------------------------------------------------- invariants and edge cases
+def test_determinism_and_member_independence(B):
+    C0 = inputs.initial_state(range(2000, 2008), 256, 2, -0.4, 0.05)
+    a, sa = run_gpu(B, C0, 1.0, 0.01, 200, 50)
+    b, sb = run_gpu(B, C0, 1.0, 0.01, 200, 50)
+    assert np.array_equal(a, b) and np.array_equal(sa, sb)            # run to run
+    p, sp = run_gpu(B, C0[::-1].copy(), 1.0, 0.01, 200, 50)
+    assert np.array_equal(p[::-1], a) and np.array_equal(sp[:, ::-1], sa)   # member position
+    one, s1 = run_gpu(B, C0[3:4].copy(), 1.0, 0.01, 200, 50)
+    assert np.array_equal(one[0], a[3]) and np.array_equal(s1[:, 0], sa[:, 3])   # ensemble size
+
+
+def test_equivariances_on_gpu(B):
+    C0 = inputs.initial_state([3, 4], 128, 2, [0.0, -0.3], 0.2)
+    base, _ = run_gpu(B, C0, 1.0, 0.01, 50, 50)
+    sh, _ = run_gpu(B, np.roll(C0, (37, -70), axis=(1, 2)).copy(), 1.0, 0.01, 50, 50)   # straddles tiles and chunks
+    assert np.abs(np.roll(sh, (-37, 70), axis=(1, 2)) - base).max() <= 1e-13
+    neg, _ = run_gpu(B, -C0, 1.0, 0.01, 50, 50)
+    assert np.array_equal(neg, -base)
+    tr, _ = run_gpu(B, np.ascontiguousarray(C0.transpose(0, 2, 1)), 1.0, 0.01, 50, 50)
+    assert np.abs(tr.transpose(0, 2, 1) - base).max() <= 1e-13
+
+
+def test_steady_state_and_split_calls(B, oracle):
+    e = B.Ensemble(1, 64, 2, 1.0, 0.01)
+    C0 = np.full((1, 64, 64), 0.37)
+    e.set_state(C0)
+    e.step(5)
+    assert np.array_equal(e.get_state(), C0)
+    e.close()
+    # ch_step(a) + ch_step(b) == ch_step(a + b), series included, also across a sampling step
+    C0 = inputs.initial_state([21], 64, 2, 0.0, 0.1)
+    whole, sw = run_gpu(B, C0, 1.0, 0.01, 60, 10)
+    e = B.Ensemble(1, 64, 2, 1.0, 0.01)
+    e.set_state(C0)
+    e.set_series(10, 7)
+    for k in (0, 7, 3, 10, 25, 15):
+        e.step(k)
+    assert np.array_equal(e.get_state(), whole) and np.array_equal(e.series(), sw)
+    assert B.ch_step_count(e.ctx) == 60 and B.ch_series_count(e.ctx) == 7
+    e.close()
+
+
+def test_errors_and_edge_cases(B):
+    e = B.Ensemble(1, 16, 2, 1.0, 0.01)
+    with pytest.raises(B.ChError) as ei:
+        e.step(1)
+    assert ei.value.code == B.CH_ESTATE
+    with pytest.raises(B.ChError):
+        e.energy()
+    C0 = inputs.initial_state([1], 16, 2, 0.0, 0.1)
+    e.set_state(C0)
+    with pytest.raises(B.ChError) as ei:
+        B.ch_step(e.ctx, -1)
+    assert ei.value.code == B.CH_EINVAL
+    e.set_series(5, 2)
+    e.step(5)                                   # samples n = 0 and n = 5: exactly full
+    with pytest.raises(B.ChError) as ei:
+        e.step(5)                               # would need a third sample
+    assert ei.value.code == B.CH_EINVAL and "series full" in str(ei.value)
+    assert B.ch_step_count(e.ctx) == 5          # nothing was enqueued
+    e.step(4)                                   # no new sample needed
+    bad = C0.copy()
+    bad[0, 3, 3] = np.nan
+    e.set_state(bad)
+    with pytest.raises(B.ChError) as ei:
+        e.energy()
+    assert ei.value.code == B.CH_ENONFINITE
+    with pytest.raises(B.ChError):
+        B.ch_set_option(e.ctx, "nonsense", 1)
+    e.close()
+
+
+def test_attached_workspace_and_device_pointers(B):
+    import torch
+    M, N = 4, 64
+    C0 = inputs.initial_state(range(M), N, 2, 0.0, 0.1)
+    ref, sref = run_gpu(B, C0, 1.0, 0.01, 40, 10)
+    ws = torch.empty(B.ch_workspace_bytes(M, N, 2), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.Stream()
+    e = B.Ensemble(M, N, 2, 1.0, 0.01, stream=stream.cuda_stream)
+    B.ch_attach_workspace(e.ctx, ws)
+    with torch.cuda.stream(stream):
+        d = torch.from_numpy(C0).cuda()
+    stream.synchronize()
+    e.set_state(d)
+    e.set_series(10, 5)
+    e.step(40)
+    out = torch.empty_like(d)
+    B.ch_get_state(e.ctx, out)
+    en = torch.empty((M, 4), dtype=torch.float64, device="cuda")
+    B.ch_energy(e.ctx, en)
+    stream.synchronize()
+    assert np.array_equal(out.cpu().numpy(), ref)
+    assert np.array_equal(e.series(), sref)
+    assert np.array_equal(en.cpu().numpy(), sref[-1])
+    assert B.ch_launch_count(e.ctx) > 0
+    e.close()
