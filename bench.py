@@ -252,7 +252,10 @@ def run_ours(args):
 
     ens.close()
     if rank == 0:
-        cpu = oracle_sample(name, max(5, int(1.5e8 / N ** D)))    # ~10-20 s of CPU work per core
+        if args.no_cpu_baseline:      # profiling runs (ncu) only: skip the CPU leg
+            cpu = {"value": None, "unit": UNIT, "cores": 0, "kind": "oracle", "sample": "skipped (--no-cpu-baseline)"}
+        else:
+            cpu = oracle_sample(name, max(5, int(1.5e8 / N ** D)))    # ~10-20 s of CPU work per core
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": secs / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -276,6 +279,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--workload", default="cfg3", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (for runs under ncu)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
