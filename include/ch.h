@@ -123,15 +123,20 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
 
 /* Kernel-variant options (measurement knobs; every variant computes the same step):
  *   "sweep"   0 auto, 1 force the generic thread-per-line sweeps, 2 force the chunked sweeps
+ *   "fuse"    0 auto (D = 2, N % 16 == 0: the fused step -- RHS fused into the y-sweep, then the x-sweep
+ *             fused with C += w; 40 instead of 56 bytes per grid-point update), 1 force the three-pass
+ *             step (RHS, x-sweep, y-sweep + update), 2 require the fused step
  * ch_get_option also answers "chunked" (chunk length of the fast sweeps, 0 if N needs the
- * generic path) and "K" (chunk neighbours summed by the periodic closure). */
+ * generic path), "K" (chunk neighbours summed by the periodic closure) and "fused" (thread-block
+ * cluster size of the fused 2D step, 0 if this shape has none). */
 int ch_set_option(ch_ctx *ctx, const char *key, int value);
 int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
 
 /* Per-kernel device timing.  ch_profile(ctx, 1) makes every later launch be bracketed by CUDA
  * events on the context's stream; ch_profile_read synchronises, returns the summed milliseconds
  * and launch counts per kernel kind (ch_kernel_kinds() kinds, named by ch_kernel_kind_name:
- * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z) and clears the records. */
+ * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z, rhs_sweep_y, rhs_sweep_y_diag, sweep_x_update)
+ * and clears the records. */
 int ch_profile(ch_ctx *ctx, int enable);
 int ch_profile_read(ch_ctx *ctx, double *ms, long long *counts, int nkinds);
 int ch_kernel_kinds(void);

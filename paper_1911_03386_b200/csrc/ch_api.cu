@@ -10,9 +10,12 @@
 #include "../../include/ch.h"
 #include "ch_factor.h"
 #include "ch_kernels.cuh"
+#include "ch_fused2d.cuh"
 
-enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z, KIND_COUNT };
-static const char *const kKindNames[KIND_COUNT] = { "rhs", "rhs_diag", "finish", "sweep_x", "sweep_y", "sweep_z" };
+enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z,
+       KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_COUNT };
+static const char *const kKindNames[KIND_COUNT] = { "rhs", "rhs_diag", "finish", "sweep_x", "sweep_y", "sweep_z",
+                                                    "rhs_sweep_y", "rhs_sweep_y_diag", "sweep_x_update" };
 
 struct ProfRec { int kind; cudaEvent_t e0, e1; };
 
@@ -45,6 +48,10 @@ struct ch_ctx {
     cudaStream_t stream;
     // options
     int opt_sweep;          // 0 auto, 1 generic, 2 chunked
+    int opt_fuse;           // 0 auto (fused 2D step when available), 1 off, 2 on
+    // fused 2D step (ch_fused2d.cuh)
+    bool fused_ok;
+    int f_CPB, f_CS, f_strips;   // chunks per CTA, CTAs per cluster, column strips per member
     long long launches;
     bool profiling;
     std::vector<ProfRec> prof;
@@ -84,6 +91,7 @@ static int fail(ch_ctx *ctx, int code, const std::string &msg)
             return fail(ctx, CH_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
     } while (0)
 
+static int chunk_len_for(int N);
 static size_t ipow(size_t n, int d) { size_t p = 1; while (d-- > 0) p *= n; return p; }
 static size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
@@ -93,13 +101,36 @@ static int rhs_parts(int N, int D)
     return ((N + RHS3_TX - 1) / RHS3_TX) * ((N + RHS3_TY - 1) / RHS3_TY) * ((N + RHS3_TZ - 1) / RHS3_TZ);
 }
 
+// Fused 2D step geometry: chunks per CTA (CPB) and cluster size (CS) for P chunks per line.
+// Returns false when no legal split exists (then the three-pass path is used).
+static bool fused_geometry(int N, int D, int *CPB, int *CS, int *strips)
+{
+    const int LC = chunk_len_for(N);
+    if (D != 2 || LC == 0) return false;
+    const int P = N / LC;
+    if (P > 64) return false;                      // exchange slots: 4 * P * 32 doubles of shared memory
+    int best = 0;
+    for (int cpb = 1; cpb <= 16 && cpb <= P; ++cpb)
+        if (P % cpb == 0 && P / cpb <= 8) { best = cpb; if (cpb >= 8) break; }
+    if (!best) return false;
+    *CPB = best; *CS = P / best; *strips = (N + FUSED_VALID - 1) / FUSED_VALID;
+    return true;
+}
+
+static int max_parts(int N, int D)
+{
+    int n = rhs_parts(N, D), cpb, cs, st;
+    if (fused_geometry(N, D, &cpb, &cs, &st) && st * cs > n) n = st * cs;
+    return n;
+}
+
 static bool shape_ok(int ensemble, int N, int D) { return ensemble >= 1 && N >= 8 && (D == 2 || D == 3); }
 
 extern "C" size_t ch_workspace_bytes(int ensemble, int N, int D)
 {
     if (!shape_ok(ensemble, N, D)) return 0;
     const size_t total = (size_t)ensemble * ipow(N, D);
-    return 2 * align256(total * 8) + align256((size_t)ensemble * rhs_parts(N, D) * 3 * 8) + align256((size_t)ensemble * 4 * 8);
+    return 2 * align256(total * 8) + align256((size_t)ensemble * max_parts(N, D) * 3 * 8) + align256((size_t)ensemble * 4 * 8);
 }
 
 static void carve(ch_ctx *c)
@@ -107,7 +138,7 @@ static void carve(ch_ctx *c)
     char *p = (char *)c->ws_base;
     c->C = (double *)p; p += align256(c->total * 8);
     c->w = (double *)p; p += align256(c->total * 8);
-    c->partials = (double *)p; p += align256((size_t)c->M * c->nparts * 3 * 8);
+    c->partials = (double *)p; p += align256((size_t)c->M * max_parts(c->N, c->D) * 3 * 8);
     c->eout = (double *)p;
 }
 
@@ -152,7 +183,9 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->C = c->w = c->partials = c->eout = nullptr;
     c->has_state = false; c->n = 0; c->t0 = 0.0;
     c->series = nullptr; c->stride = 0; c->capacity = 0; c->cursor = 0; c->last_sampled = -1;
-    c->stream = 0; c->opt_sweep = 0; c->launches = 0; c->profiling = false;
+    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->launches = 0; c->profiling = false;
+    c->f_CPB = c->f_CS = c->f_strips = 0;
+    c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
     if (c->chunked) {
         cudaError_t e = cudaMalloc((void **)&c->dW, sizeof(double) * 4 * CH_MAX_P);
         if (e == cudaSuccess) e = cudaMemcpy(c->dW, c->fac.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
@@ -174,6 +207,12 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     cudaFuncSetAttribute(k_sweep_contig<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
     cudaFuncSetAttribute(k_sweep_contig<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
     cudaFuncSetAttribute(k_sweep_contig<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaFuncSetAttribute(k_rhs_sweep_y<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaFuncSetAttribute(k_rhs_sweep_y<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaFuncSetAttribute(k_rhs_sweep_y<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaFuncSetAttribute(k_rhs_sweep_y<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaFuncSetAttribute(k_sweep_x_update<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_sweep_x_update<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaGetLastError();
     *out = c;
     return CH_OK;
@@ -298,6 +337,12 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_sweep = value;
         return CH_OK;
     }
+    if (!strcmp(key, "fuse")) {
+        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0, 1 or 2");
+        if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the fused step needs D = 2 and N % 16 == 0");
+        ctx->opt_fuse = value;
+        return CH_OK;
+    }
     return fail(ctx, CH_EINVAL, std::string("ch_set_option: unknown option ") + key);
 }
 
@@ -307,6 +352,8 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "sweep")) { *value = ctx->opt_sweep; return CH_OK; }
     if (!strcmp(key, "chunked")) { *value = ctx->chunked ? ctx->LC : 0; return CH_OK; }
     if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
+    if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
+    if (!strcmp(key, "fused")) { *value = ctx->fused_ok ? ctx->f_CS : 0; return CH_OK; }
     return CH_EINVAL;
 }
 
@@ -335,10 +382,10 @@ static void launch_rhs(ch_ctx *c, const double *C, double *r, double scale, bool
     else launch_rhs_t<false, true>(c, C, r, scale);
 }
 
-static void launch_finish(ch_ctx *c, double *out, double t)
+static void launch_finish(ch_ctx *c, double *out, double t, int nparts)
 {
     ProfScope ps(c, KIND_FINISH);
-    k_finish<<<c->M, 128, 0, c->stream>>>(c->partials, c->nparts, out, t);
+    k_finish<<<c->M, 128, 0, c->stream>>>(c->partials, nparts, out, t);
 }
 
 static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
@@ -409,6 +456,62 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
 #undef LAUNCH_STRIDED
 }
 
+static bool use_fused(const ch_ctx *c) { return c->fused_ok && c->opt_fuse != 1 && c->opt_sweep != 1; }
+
+// ---- fused 2D step: (RHS + y-sweep) then (x-sweep + update) ------------------------------------
+template <int LC, bool DIAG>
+static void launch_rhs_sweep_y_t(ch_ctx *c, const SweepParams &prm, int write)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((size_t)c->f_CS * c->f_strips * c->M));
+    cfg.blockDim = dim3(32, c->f_CPB);
+    cfg.dynamicSmemBytes = (size_t)4 * c->fac.P * 32 * 8;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = c->f_CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_rhs_sweep_y<LC, DIAG>, prm, (const double *)c->C, c->w, c->partials, c->N, c->gamma,
+                       c->rscale, c->f_strips, c->f_CS, write);
+}
+
+// diag: also reduce F, Fdot, mass of C^n into the partials; write == false (diag only): no sweep, w untouched
+static void launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
+{
+    ProfScope ps(c, diag ? KIND_RHS_SWEEP_Y_DIAG : KIND_RHS_SWEEP_Y);
+    SweepParams prm;
+    fill_params(c, prm, 1.0);
+    if (c->LC == 16) { if (diag) launch_rhs_sweep_y_t<16, true>(c, prm, write); else launch_rhs_sweep_y_t<16, false>(c, prm, 1); }
+    else { if (diag) launch_rhs_sweep_y_t<32, true>(c, prm, write); else launch_rhs_sweep_y_t<32, false>(c, prm, 1); }
+}
+
+// F, Fdot, mass partials of the current state with the same kernel (hence the same summation order)
+// the stepping path samples with, so that splitting ch_step calls never changes a series value.
+static int launch_diag_only(ch_ctx *c)
+{
+    if (use_fused(c)) { launch_rhs_sweep_y(c, true, false); return c->f_strips * c->f_CS; }
+    launch_rhs(c, c->C, c->w, c->rscale, true, false);
+    return c->nparts;
+}
+
+static void launch_sweep_x_update(ch_ctx *c)
+{
+    ProfScope ps(c, KIND_SWEEP_X_UPDATE);
+    SweepParams prm;
+    fill_params(c, prm, 1.0);
+    const int N = c->N, P = c->fac.P;
+    const long long total_lines = (long long)c->M * N;
+    int threads = 256;
+    if (P > threads) threads = P;
+    int LPB = threads / P;
+    if (LPB > total_lines) LPB = (int)total_lines;
+    threads = LPB * P;
+    const int blocks = (int)((total_lines + LPB - 1) / LPB);
+    const size_t smem = (size_t)2 * LPB * N * 8 + (size_t)2 * LPB * P * 8;
+    if (c->LC == 16) k_sweep_x_update<16><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
+    else k_sweep_x_update<32><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
+}
+
 static int check_launch(ch_ctx *ctx, const char *what)
 {
     cudaError_t e = cudaGetLastError();
@@ -430,19 +533,23 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
         if (ctx->cursor + cnt > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_step: series full");
     }
     const int D = ctx->D;
+    const bool fused = use_fused(ctx);
     for (int s = 0; s < nsteps; ++s) {
         const bool sample = ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n;
-        launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
+        if (fused) launch_rhs_sweep_y(ctx, sample, true);
+        else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
         if (sample) {
-            launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt);
+            launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
+                          fused ? ctx->f_strips * ctx->f_CS : ctx->nparts);
             ctx->cursor++; ctx->last_sampled = ctx->n;
         }
-        for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
+        if (fused) launch_sweep_x_update(ctx);
+        else for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
         ctx->n++;
     }
     if (ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n) {
-        launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, true, false);
-        launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt);
+        const int np_ = launch_diag_only(ctx);
+        launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt, np_);
         ctx->cursor++; ctx->last_sampled = ctx->n;
     }
     return check_launch(ctx, "ch_step");
@@ -454,8 +561,8 @@ extern "C" int ch_energy(ch_ctx *ctx, double *out, int on_device)
     if (!out) return fail(ctx, CH_EINVAL, "ch_energy: out is NULL");
     if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_energy: no state");
     const double t = ctx->t0 + (double)ctx->n * ctx->dt;
-    launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, true, false);
-    launch_finish(ctx, on_device ? out : ctx->eout, t);
+    const int np_ = launch_diag_only(ctx);
+    launch_finish(ctx, on_device ? out : ctx->eout, t, np_);
     int rc = check_launch(ctx, "ch_energy");
     if (rc) return rc;
     if (!on_device) {

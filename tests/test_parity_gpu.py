@@ -216,6 +216,27 @@ def test_generic_paths_end_to_end(B, oracle):
         assert_series_close(s, so)
 
 
+@pytest.mark.parametrize("N", [16, 48, 64, 80, 176, 256, 592, 1024])
+@pytest.mark.parametrize("gamma,dt", [(1.0, 0.01), (66.4, 7.97)])
+def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
+    """The fused 2D step (RHS + y-sweep, then x-sweep + update; cluster sizes 1..8, ragged last
+    column strip) and the three-pass step against the oracle and each other; N = 592 (37 chunks per
+    line) has no legal cluster split and must fall back to three passes by itself."""
+    M = 2 if N <= 256 else 1
+    nsteps = 100 if N <= 256 else 20
+    C0 = inputs.initial_state([5, 6][:M], N, 2, [0.0, -0.4][:M], 0.1)
+    Co, so = oracle.run(C0, gamma, dt, nsteps, 10)
+    tol, rtol = (FIELD_TOL, SERIES_RTOL) if gamma == 1.0 else (1e-9, 1e-7)
+    e = B.Ensemble(M, N, 2, gamma, dt)
+    cs = B.ch_get_option(e.ctx, "fused")
+    e.close()
+    assert (cs == 0) == (N == 592)
+    for opts in ([None, {"fuse": 1}] if cs else [None]):
+        C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options=opts)
+        assert np.abs(C - Co).max() <= tol, (N, opts)
+        assert_series_close(s, so, rtol)
+
+
 # ---------------------------------------------------- invariants and edge cases
 def test_determinism_and_member_independence(B):
     C0 = inputs.initial_state(range(2000, 2008), 256, 2, -0.4, 0.05)
