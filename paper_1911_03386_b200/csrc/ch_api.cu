@@ -465,7 +465,7 @@ static void launch_rhs_sweep_y_t(ch_ctx *c, const SweepParams &prm, int write)
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)((size_t)c->f_CS * c->f_strips * c->M));
     cfg.blockDim = dim3(32, c->f_CPB);
-    cfg.dynamicSmemBytes = (size_t)4 * c->fac.P * 32 * 8;
+    cfg.dynamicSmemBytes = (size_t)2 * c->fac.P * 32 * 16;
     cfg.stream = c->stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;

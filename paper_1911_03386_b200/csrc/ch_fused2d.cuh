@@ -20,13 +20,84 @@ namespace cg = cooperative_groups;
 #define FUSED_VALID 28        // columns a warp produces: 32 lanes minus a halo of 2 on either side
 
 // ------------------------------------------------------------------------------------
+// Distributed-shared-memory plumbing (sm_90+ PTX): cluster barrier split into arrive / wait,
+// mbarrier with a transaction count, and st.async -- a remote shared-memory store that signals
+// the receiving CTA's mbarrier when it lands, so the chunk-state exchange needs no fences.
+// ------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned mbar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(mbar), "r"(parity) : "memory");
+}
+// address of the same shared-memory location in CTA `rank` of the cluster
+__device__ __forceinline__ unsigned map_rank(unsigned local, unsigned rank)
+{
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(local), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_async_2f64(unsigned remote_addr, double a, double b, unsigned remote_mbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];\n" ::"r"(remote_addr),
+                 "l"(__double_as_longlong(a)), "l"(__double_as_longlong(b)), "r"(remote_mbar)
+                 : "memory");
+}
+
+// read-only global load as volatile asm: keeps the compiler from sinking it below later code, so a
+// thread's loads are all in flight together
+__device__ __forceinline__ double ldg_nc_f64(const double *p)
+{
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];\n" : "=d"(v) : "l"(p));
+    return v;
+}
+
+// state entering chunk c from the K chunks before it (dir = +1) or after it (dir = -1); slots hold
+// (a, b) pairs indexed [chunk][lane]
+__device__ __forceinline__ void chunk_state_in2(const SweepParams &prm, const double2 *slots, int c, int lane, int dir,
+                                                double &a, double &b)
+{
+    a = 0.0; b = 0.0;
+    const int P = prm.P;
+    int s = c;
+    for (int j = 0; j < prm.K; ++j) {
+        s -= dir;
+        if (s < 0) s += P;
+        if (s >= P) s -= P;
+        const double2 o = slots[s * 32 + lane];
+        const double2 W01 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j);
+        const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
+        a = fma(W01.x, o.x, fma(W01.y, o.y, a));
+        b = fma(W23.x, o.x, fma(W23.y, o.y, b));
+    }
+}
+
+// ------------------------------------------------------------------------------------
 // k_rhs_sweep_y.  One warp = 32 adjacent columns (28 produced + 2 halo lanes each side, x-neighbours
 // by warp shuffle), thread (lane, cl) marches down the LC rows of chunk c = crank * CPB + cl.
 // A thread-block cluster of CS = P / CPB CTAs covers the whole column strip; the 2-double chunk
-// out-states are pushed into every CTA of the cluster through distributed shared memory, so the
-// periodic closure (ch_factor.h) sees all P chunks of a line.
+// out-states are pushed into every CTA of the cluster with st.async (distributed shared memory +
+// mbarrier transaction counts), so the periodic closure (ch_factor.h) sees all P chunks of a line.
 // grid.x = CS * strips * ensemble (cluster dim x = CS), block = (32, CPB).
-// dynamic smem = 4 * P * 32 doubles: sa_f, sb_f, sa_b, sb_b indexed [chunk][lane].
+// dynamic smem = 2 * P * 32 double2: forward and backward exchange slots, indexed [chunk][lane].
 // ------------------------------------------------------------------------------------
 template <int LC, bool DIAG>
 __global__ void __launch_bounds__(512) k_rhs_sweep_y(const __grid_constant__ SweepParams prm,
@@ -34,9 +105,9 @@ __global__ void __launch_bounds__(512) k_rhs_sweep_y(const __grid_constant__ Swe
                                                      double *__restrict__ partials, int N, double gamma, double scale,
                                                      int strips, int CS, int write)
 {
-    extern __shared__ double sx[];
+    extern __shared__ double2 sx2[];
     __shared__ double red[16][3];
-    cg::cluster_group cluster = cg::this_cluster();
+    __shared__ __align__(8) unsigned long long mbar[2];
     const int lane = threadIdx.x, cl = threadIdx.y, CPB = blockDim.y, P = prm.P;
     const int crank = blockIdx.x % CS, tile = blockIdx.x / CS;
     const int strip = tile % strips, m = tile / strips;
@@ -47,17 +118,31 @@ __global__ void __launch_bounds__(512) k_rhs_sweep_y(const __grid_constant__ Swe
     while (gx >= N) gx -= N;
     const bool valid = lane >= 2 && lane < 30 && (X + lane - 2) < N;
     const int y0 = c * LC;
-    const double *Cm = C + (size_t)m * N * N + gx;
+    const size_t n2 = (size_t)N * N;
 
-    // C rows y0-2 .. y0+LC+1 of this thread's column (periodic in y)
-    double cv[LC + 4];
-#pragma unroll
-    for (int j = 0; j < LC + 4; ++j) {
-        int y = y0 - 2 + j;
-        if (y < 0) y += N;
-        if (y >= N) y -= N;
-        cv[j] = __ldg(Cm + (size_t)y * N);
+    const unsigned mb_f = smem_u32(&mbar[0]), mb_b = smem_u32(&mbar[1]);
+    if (lane == 0 && cl == 0) {
+        mbar_init(mb_f, 1);
+        mbar_init(mb_b, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        mbar_expect_tx(mb_f, (unsigned)P * 32 * 16);
+        mbar_expect_tx(mb_b, (unsigned)P * 32 * 16);
     }
+    cluster_arrive();        // waited on just before the first remote store, long after every CTA has started
+
+    // C rows y0-2 .. y0+LC+1 of this thread's column; only the two halo rows on either end can wrap
+    double cv[LC + 4];
+    {
+        const double *p = C + (size_t)m * n2 + gx + (ptrdiff_t)(y0 - 2) * N;
+        const double *plo = (c == 0) ? p + n2 : p;
+        const double *phi = (c == P - 1) ? p - n2 : p;
+#pragma unroll
+        for (int j = 0; j < LC + 4; ++j) {
+            const double *q = (j < 2) ? plo : ((j >= LC + 2) ? phi : p);
+            cv[j] = ldg_nc_f64(q + (ptrdiff_t)j * N);
+        }
+    }
+    asm volatile("" ::: "memory");    // all LC+4 loads are issued before any arithmetic (keeps them in flight together)
 
     double v[LC];
     double F = 0.0, Fd = 0.0, ms = 0.0;
@@ -112,35 +197,28 @@ __global__ void __launch_bounds__(512) k_rhs_sweep_y(const __grid_constant__ Swe
             o[0] = F; o[1] = Fd; o[2] = ms;
         }
     }
+    cluster_wait();                   // every CTA of the cluster has initialised its mbarriers
     if (DIAG && !write) return;       // diagnostics only (grid-uniform): no sweep, no cluster traffic
 
-    double *sa_f = sx, *sb_f = sx + P * 32, *sa_b = sx + 2 * P * 32, *sb_b = sx + 3 * P * 32;
-    cluster.sync();                                     // every CTA of the cluster is resident
-    for (int rk = 0; rk < CS; ++rk) {
-        double *ra = cluster.map_shared_rank(sa_f, rk), *rb = cluster.map_shared_rank(sb_f, rk);
-        ra[c * 32 + lane] = v[LC - 1];
-        rb[c * 32 + lane] = v[LC - 2];
-    }
-    cluster.sync();
+    double2 *sf = sx2, *sb = sx2 + P * 32;
+    const unsigned slot_f = smem_u32(sf + c * 32 + lane), slot_b = smem_u32(sb + c * 32 + lane);
+    for (int rk = 0; rk < CS; ++rk) st_async_2f64(map_rank(slot_f, rk), v[LC - 1], v[LC - 2], map_rank(mb_f, rk));
+    mbar_wait(mb_f, 0);
     double a, b;
-    chunk_state_in<LC>(prm, sa_f + lane, sb_f + lane, c, 32, +1, a, b);
+    chunk_state_in2(prm, sf, c, lane, +1, a, b);
 #pragma unroll
     for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
     // backward recurrence from a zero state
     v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
 #pragma unroll
     for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
-    for (int rk = 0; rk < CS; ++rk) {
-        double *ra = cluster.map_shared_rank(sa_b, rk), *rb = cluster.map_shared_rank(sb_b, rk);
-        ra[c * 32 + lane] = v[0];
-        rb[c * 32 + lane] = v[1];
-    }
-    cluster.sync();                                     // after this nobody touches remote smem again
-    chunk_state_in<LC>(prm, sa_b + lane, sb_b + lane, c, 32, -1, a, b);
+    for (int rk = 0; rk < CS; ++rk) st_async_2f64(map_rank(slot_b, rk), v[0], v[1], map_rank(mb_b, rk));
+    mbar_wait(mb_b, 0);               // all P chunk states have landed here: nobody writes this CTA again
+    chunk_state_in2(prm, sb, c, lane, -1, a, b);
     if (valid) {
-        double *wm = w + (size_t)m * N * N + (size_t)y0 * N + gx;
+        double *wm = w + (size_t)m * n2 + (size_t)y0 * N + gx;
 #pragma unroll
-        for (int k = 0; k < LC; ++k) wm[(size_t)k * N] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
+        for (int k = 0; k < LC; ++k) wm[(ptrdiff_t)k * N] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
     }
 }
 
