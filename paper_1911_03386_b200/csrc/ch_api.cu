@@ -11,6 +11,7 @@
 #include "ch_factor.h"
 #include "ch_kernels.cuh"
 #include "ch_fused2d.cuh"
+#include "ch_line2d.cuh"
 
 enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z,
        KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_COUNT };
@@ -48,15 +49,27 @@ struct ch_ctx {
     cudaStream_t stream;
     // options
     int opt_sweep;          // 0 auto, 1 generic, 2 chunked
-    int opt_fuse;           // 0 auto (fused 2D step when available), 1 off, 2 on
+    int opt_fuse;           // 0 auto (fused 2D step when available), 1 off, 2 cluster kernel, 3 line kernel
     // fused 2D step (ch_fused2d.cuh)
     bool fused_ok;
     int f_CPB, f_CS, f_strips;   // chunks per CTA, CTAs per cluster, column strips per member
+    // fused 2D step, whole line in one CTA (ch_line2d.cuh)
+    bool line_ok;
+    int l_strips, l_resident;    // column strips per member, CTAs resident on the device
     long long launches;
     bool profiling;
     std::vector<ProfRec> prof;
     std::string err;
 };
+
+// which fused 2D step runs: 0 none (three-pass), 2 cluster kernel, 3 line kernel
+static int fuse_mode(const ch_ctx *c)
+{
+    if (c->opt_fuse == 1 || c->opt_sweep == 1) return 0;
+    if (c->opt_fuse == 2) return c->fused_ok ? 2 : 0;
+    if (c->opt_fuse == 3) return c->line_ok ? 3 : 0;
+    return c->line_ok ? 3 : (c->fused_ok ? 2 : 0);
+}
 
 // Brackets one kernel launch with CUDA events on the context's stream when profiling is on.
 struct ProfScope {
@@ -117,10 +130,25 @@ static bool fused_geometry(int N, int D, int *CPB, int *CS, int *strips)
     return true;
 }
 
+// Line kernel geometry: whole lines of P = N / 16 chunks in one CTA of 16 P threads.
+static bool line_geometry(int N, int D, int *strips)
+{
+    if (D != 2 || N % (2 * LINE_LC) != 0 || N / LINE_LC > LINE_MAX_P) return false;
+    *strips = (N + LINE_VALID - 1) / LINE_VALID;
+    return true;
+}
+
+static size_t line_smem(int N)
+{
+    const int P = N / LINE_LC;
+    return (size_t)(LINE_LC + 4) * 16 * P * 16 + (size_t)4 * P * 16 * 16;
+}
+
 static int max_parts(int N, int D)
 {
     int n = rhs_parts(N, D), cpb, cs, st;
     if (fused_geometry(N, D, &cpb, &cs, &st) && st * cs > n) n = st * cs;
+    if (line_geometry(N, D, &st) && st > n) n = st;
     return n;
 }
 
@@ -186,6 +214,8 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->launches = 0; c->profiling = false;
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
+    c->l_strips = 0; c->l_resident = 0;
+    c->line_ok = line_geometry(N, D, &c->l_strips);
     if (c->chunked) {
         cudaError_t e = cudaMalloc((void **)&c->dW, sizeof(double) * 4 * CH_MAX_P);
         if (e == cudaSuccess) e = cudaMemcpy(c->dW, c->fac.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
@@ -213,6 +243,17 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     cudaFuncSetAttribute(k_rhs_sweep_y<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     cudaFuncSetAttribute(k_sweep_x_update<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_sweep_x_update<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (c->line_ok) {
+        const int smem = (int)line_smem(N);
+        int per_sm = 0, dev = 0, sms = 0;
+        cudaError_t e = cudaFuncSetAttribute(k_rhs_sweep_y_line<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_rhs_sweep_y_line<true>, N, smem);
+        if (e == cudaSuccess) e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || per_sm < 1 || sms < 1) c->line_ok = false;
+        else c->l_resident = per_sm * sms;
+    }
     cudaGetLastError();
     *out = c;
     return CH_OK;
@@ -338,8 +379,9 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         return CH_OK;
     }
     if (!strcmp(key, "fuse")) {
-        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0, 1 or 2");
-        if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the fused step needs D = 2 and N % 16 == 0");
+        if (value < 0 || value > 3) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster) or 3 (line)");
+        if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
+        if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2, N % 32 == 0 and N <= 512");
         ctx->opt_fuse = value;
         return CH_OK;
     }
@@ -354,6 +396,8 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
     if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
     if (!strcmp(key, "fused")) { *value = ctx->fused_ok ? ctx->f_CS : 0; return CH_OK; }
+    if (!strcmp(key, "line")) { *value = ctx->line_ok ? ctx->l_resident : 0; return CH_OK; }
+    if (!strcmp(key, "fuse_mode")) { *value = fuse_mode(ctx); return CH_OK; }
     return CH_EINVAL;
 }
 
@@ -456,7 +500,7 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
 #undef LAUNCH_STRIDED
 }
 
-static bool use_fused(const ch_ctx *c) { return c->fused_ok && c->opt_fuse != 1 && c->opt_sweep != 1; }
+static bool use_fused(const ch_ctx *c) { return fuse_mode(c) != 0; }
 
 // ---- fused 2D step: (RHS + y-sweep) then (x-sweep + update) ------------------------------------
 template <int LC, bool DIAG>
@@ -475,10 +519,29 @@ static void launch_rhs_sweep_y_t(ch_ctx *c, const SweepParams &prm, int write)
                        c->rscale, c->f_strips, c->f_CS, write);
 }
 
+static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
+{
+    LineParams p;
+    p.np = c->fac.np; p.nq = c->fac.nq;
+    p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0; p.scale = c->rscale;
+    memcpy(p.alpha, c->fac.alpha, sizeof(p.alpha));
+    memcpy(p.beta, c->fac.beta, sizeof(p.beta));
+    p.W = c->dW; p.K = c->fac.K; p.P = c->fac.P; p.N = c->N;
+    p.strips = c->l_strips; p.ntiles = c->l_strips * c->M; p.write = write ? 1 : 0;
+    const int grid = p.ntiles < c->l_resident ? p.ntiles : c->l_resident;
+    const size_t smem = line_smem(c->N);
+    if (diag) k_rhs_sweep_y_line<true><<<grid, 16 * p.P, smem, c->stream>>>(p, c->C, c->w, c->partials);
+    else k_rhs_sweep_y_line<false><<<grid, 16 * p.P, smem, c->stream>>>(p, c->C, c->w, c->partials);
+}
+
+// number of F/Fdot/mass partials per member the fused RHS kernel in use writes
+static int fused_parts(const ch_ctx *c) { return fuse_mode(c) == 3 ? c->l_strips : c->f_strips * c->f_CS; }
+
 // diag: also reduce F, Fdot, mass of C^n into the partials; write == false (diag only): no sweep, w untouched
 static void launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
 {
     ProfScope ps(c, diag ? KIND_RHS_SWEEP_Y_DIAG : KIND_RHS_SWEEP_Y);
+    if (fuse_mode(c) == 3) { launch_rhs_sweep_y_line(c, diag, write); return; }
     SweepParams prm;
     fill_params(c, prm, 1.0);
     if (c->LC == 16) { if (diag) launch_rhs_sweep_y_t<16, true>(c, prm, write); else launch_rhs_sweep_y_t<16, false>(c, prm, 1); }
@@ -489,7 +552,7 @@ static void launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
 // the stepping path samples with, so that splitting ch_step calls never changes a series value.
 static int launch_diag_only(ch_ctx *c)
 {
-    if (use_fused(c)) { launch_rhs_sweep_y(c, true, false); return c->f_strips * c->f_CS; }
+    if (use_fused(c)) { launch_rhs_sweep_y(c, true, false); return fused_parts(c); }
     launch_rhs(c, c->C, c->w, c->rscale, true, false);
     return c->nparts;
 }
@@ -540,7 +603,7 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
         else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
         if (sample) {
             launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
-                          fused ? ctx->f_strips * ctx->f_CS : ctx->nparts);
+                          fused ? fused_parts(ctx) : ctx->nparts);
             ctx->cursor++; ctx->last_sampled = ctx->n;
         }
         if (fused) launch_sweep_x_update(ctx);

@@ -216,25 +216,44 @@ def test_generic_paths_end_to_end(B, oracle):
         assert_series_close(s, so)
 
 
-@pytest.mark.parametrize("N", [16, 48, 64, 80, 176, 256, 592, 1024])
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 176, 256, 352, 512, 592, 1024])
 @pytest.mark.parametrize("gamma,dt", [(1.0, 0.01), (66.4, 7.97)])
 def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
-    """The fused 2D step (RHS + y-sweep, then x-sweep + update; cluster sizes 1..8, ragged last
-    column strip) and the three-pass step against the oracle and each other; N = 592 (37 chunks per
-    line) has no legal cluster split and must fall back to three passes by itself."""
+    """Every 2D step variant against the oracle: the line-fused step (RHS + y-sweep with whole lines
+    in one persistent CTA, N % 32 == 0 and N <= 512; ragged last column strip, more tiles than
+    resident CTAs at M = 40), the cluster-fused step (cluster sizes 1..8) and the three-pass step.
+    N = 592 (37 chunks per line) has no legal split and must fall back to three passes by itself."""
     M = 2 if N <= 256 else 1
     nsteps = 100 if N <= 256 else 20
     C0 = inputs.initial_state([5, 6][:M], N, 2, [0.0, -0.4][:M], 0.1)
     Co, so = oracle.run(C0, gamma, dt, nsteps, 10)
     tol, rtol = (FIELD_TOL, SERIES_RTOL) if gamma == 1.0 else (1e-9, 1e-7)
     e = B.Ensemble(M, N, 2, gamma, dt)
-    cs = B.ch_get_option(e.ctx, "fused")
+    cs, line, mode = B.ch_get_option(e.ctx, "fused"), B.ch_get_option(e.ctx, "line"), B.ch_get_option(e.ctx, "fuse_mode")
     e.close()
     assert (cs == 0) == (N == 592)
-    for opts in ([None, {"fuse": 1}] if cs else [None]):
+    assert (line != 0) == (N % 32 == 0 and N <= 512)
+    assert mode == (3 if line else (2 if cs else 0))
+    variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}] if line else [])
+    for opts in variants:
         C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options=opts)
         assert np.abs(C - Co).max() <= tol, (N, opts)
         assert_series_close(s, so, rtol)
+
+
+def test_line_kernel_persistent_tiles(B, oracle):
+    """More tiles than resident CTAs (40 members x 10 strips at N = 256): every CTA of the line kernel
+    loops over several tiles, prefetching the next one; members 0, 17 and 39 against the oracle and
+    all members against the three-pass step."""
+    C0 = inputs.initial_state(range(300, 340), 256, 2, -0.3, 0.1)
+    C, s = run_gpu(B, C0, 1.0, 0.01, 60, 20, options={"fuse": 3})
+    C3, s3 = run_gpu(B, C0, 1.0, 0.01, 60, 20, options={"fuse": 1})
+    assert np.abs(C - C3).max() <= 1e-13
+    assert_series_close(s, s3, 1e-12)
+    sub = [0, 17, 39]
+    Co, so = oracle.run(C0[sub], 1.0, 0.01, 60, 20)
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
 
 
 # ---------------------------------------------------- invariants and edge cases
