@@ -49,6 +49,7 @@ struct ch_ctx {
     cudaStream_t stream;
     // options
     int opt_sweep;          // 0 auto, 1 generic, 2 chunked
+    int opt_linesync;       // line kernel: 0 auto (neighbour-warp sync when K <= 2), 1 CTA barriers
     int opt_fuse;           // 0 auto (fused 2D step when available), 1 off, 2 cluster kernel, 3 line kernel
     // fused 2D step (ch_fused2d.cuh)
     bool fused_ok;
@@ -130,10 +131,17 @@ static bool fused_geometry(int N, int D, int *CPB, int *CS, int *strips)
     return true;
 }
 
-// Line kernel geometry: whole lines of P = N / 16 chunks in one CTA of 16 P threads.
+// Line kernel geometry: whole lines of P = N / 16 chunks in one CTA of N threads; N is a template
+// parameter of the kernel, instantiated for the sizes below.
+#define LINE_SIZES(X) X(32) X(64) X(96) X(128) X(192) X(256) X(384) X(512)
 static bool line_geometry(int N, int D, int *strips)
 {
-    if (D != 2 || N % (2 * LINE_LC) != 0 || N / LINE_LC > LINE_MAX_P) return false;
+    if (D != 2) return false;
+    bool ok = false;
+#define X(NC) ok = ok || N == NC;
+    LINE_SIZES(X)
+#undef X
+    if (!ok) return false;
     *strips = (N + LINE_VALID - 1) / LINE_VALID;
     return true;
 }
@@ -211,7 +219,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->C = c->w = c->partials = c->eout = nullptr;
     c->has_state = false; c->n = 0; c->t0 = 0.0;
     c->series = nullptr; c->stride = 0; c->capacity = 0; c->cursor = 0; c->last_sampled = -1;
-    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->launches = 0; c->profiling = false;
+    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->launches = 0; c->profiling = false;
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
     c->l_strips = 0; c->l_resident = 0;
@@ -246,9 +254,16 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     if (c->line_ok) {
         const int smem = (int)line_smem(N);
         int per_sm = 0, dev = 0, sms = 0;
-        cudaError_t e = cudaFuncSetAttribute(k_rhs_sweep_y_line<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_rhs_sweep_y_line<true>, N, smem);
+        cudaError_t e = cudaErrorInvalidValue;
+#define X(NC)                                                                                                             \
+        if (N == NC) {                                                                                                    \
+            e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);   \
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_rhs_sweep_y_line<NC, false, false>, NC, smem); \
+        }
+        LINE_SIZES(X)
+#undef X
         if (e == cudaSuccess) e = cudaGetDevice(&dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess || per_sm < 1 || sms < 1) c->line_ok = false;
@@ -378,10 +393,15 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_sweep = value;
         return CH_OK;
     }
+    if (!strcmp(key, "linesync")) {
+        if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: linesync must be 0 (auto) or 1 (CTA barriers)");
+        ctx->opt_linesync = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "fuse")) {
         if (value < 0 || value > 3) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster) or 3 (line)");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
-        if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2, N % 32 == 0 and N <= 512");
+        if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 192, 256, 384, 512}");
         ctx->opt_fuse = value;
         return CH_OK;
     }
@@ -526,12 +546,21 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
     p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0; p.scale = c->rscale;
     memcpy(p.alpha, c->fac.alpha, sizeof(p.alpha));
     memcpy(p.beta, c->fac.beta, sizeof(p.beta));
-    p.W = c->dW; p.K = c->fac.K; p.P = c->fac.P; p.N = c->N;
+    memcpy(p.W0, c->fac.W[0], sizeof(p.W0));
+    memcpy(p.W1, c->fac.W[1], sizeof(p.W1));
+    p.W = c->dW; p.K = c->fac.K;
     p.strips = c->l_strips; p.ntiles = c->l_strips * c->M; p.write = write ? 1 : 0;
     const int grid = p.ntiles < c->l_resident ? p.ntiles : c->l_resident;
     const size_t smem = line_smem(c->N);
-    if (diag) k_rhs_sweep_y_line<true><<<grid, 16 * p.P, smem, c->stream>>>(p, c->C, c->w, c->partials);
-    else k_rhs_sweep_y_line<false><<<grid, 16 * p.P, smem, c->stream>>>(p, c->C, c->w, c->partials);
+    const bool nb = p.K <= 2 && c->opt_linesync != 1;     // neighbour-warp synchronisation instead of CTA barriers
+#define X(NC)                                                                                                       \
+    if (c->N == NC) {                                                                                               \
+        if (diag) k_rhs_sweep_y_line<NC, true, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials);   \
+        else if (nb) k_rhs_sweep_y_line<NC, false, true><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
+        else k_rhs_sweep_y_line<NC, false, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials);       \
+    }
+    LINE_SIZES(X)
+#undef X
 }
 
 // number of F/Fdot/mass partials per member the fused RHS kernel in use writes

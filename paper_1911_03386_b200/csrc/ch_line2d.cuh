@@ -28,8 +28,9 @@ struct LineParams {
     double np, nq;                  // recurrence  z_i = b_i + np z_{i-1} + nq z_{i-2}
     double gamma, mgam, k1, scale;  // mu = c (c^2 + k1) - gamma * (sum of the 4 neighbours), k1 = 4 gamma - 1
     double alpha[LINE_LC], beta[LINE_LC];
+    double W0[4], W1[4];            // first two closure matrices (all of them when K <= 2)
     const double *W;                // device [K][4] (ch_factor.h)
-    int K, P, N, strips, ntiles, write;
+    int K, strips, ntiles, write;
 };
 
 __device__ __forceinline__ void line_cp_async16(void *smem_dst, const void *gsrc)
@@ -43,72 +44,113 @@ __device__ __forceinline__ void line_cp_async_wait_all() { asm volatile("cp.asyn
 __device__ __forceinline__ double hshfl_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1, 16); }
 __device__ __forceinline__ double hshfl_down(double v) { return __shfl_down_sync(0xffffffffu, v, 1, 16); }
 
+// Neighbour synchronisation (NB kernels, K <= 2): a warp holds chunks 2w and 2w+1, and with K <= 2 the
+// state entering a chunk depends on the two chunks before (forward) or after (backward) it only, i.e. on
+// the warp itself and ONE neighbouring warp.  Instead of a CTA-wide barrier each warp publishes a
+// sequence number (release) after writing its exchange slots and polls its neighbour's (acquire), so
+// the warps of a CTA drift apart and their load / fp64 / store phases overlap.
+__device__ __forceinline__ void flag_release(unsigned *flag, unsigned seq)
+{
+    asm volatile("st.release.cta.shared.u32 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(flag)), "r"(seq) : "memory");
+}
+__device__ __forceinline__ void flag_wait(const unsigned *flag, unsigned seq)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(flag);
+    unsigned v;
+    do {
+        asm volatile("ld.acquire.cta.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(a) : "memory");
+    } while (v < seq);
+}
+
 // states entering chunk c (both columns of the lane) from the K chunks before it (dir = +1) or after
 // it (dir = -1); slots are [column A|B][chunk][16 lanes] pairs (value next to the boundary, one further in)
+template <int P>
 __device__ __forceinline__ void line_state_in(const LineParams &prm, const double2 *slots, int c, int li, int dir,
                                               double &aA, double &bA, double &aB, double &bB)
 {
     aA = bA = aB = bB = 0.0;
-    const int P = prm.P;
-    int s = c;
-    for (int j = 0; j < prm.K; ++j) {
-        s -= dir;
-        if (s < 0) s += P;
-        if (s >= P) s -= P;
+    auto acc = [&](int s, double w0, double w1, double w2, double w3) {
         const double2 oA = slots[s * 16 + li], oB = slots[(P + s) * 16 + li];
+        aA = fma(w0, oA.x, fma(w1, oA.y, aA));
+        bA = fma(w2, oA.x, fma(w3, oA.y, bA));
+        aB = fma(w0, oB.x, fma(w1, oB.y, aB));
+        bB = fma(w2, oB.x, fma(w3, oB.y, bB));
+    };
+    int s = c;
+    auto next = [&]() { s -= dir; if (s < 0) s += P; if (s >= P) s -= P; };
+    if (prm.K <= 2) {                       // small gamma dt: the tables sit in the constant bank
+        next(); acc(s, prm.W0[0], prm.W0[1], prm.W0[2], prm.W0[3]);
+        if (prm.K == 2) { next(); acc(s, prm.W1[0], prm.W1[1], prm.W1[2], prm.W1[3]); }
+        return;
+    }
+    for (int j = 0; j < prm.K; ++j) {
+        next();
         const double2 W01 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j);
         const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
-        aA = fma(W01.x, oA.x, fma(W01.y, oA.y, aA));
-        bA = fma(W23.x, oA.x, fma(W23.y, oA.y, bA));
-        aB = fma(W01.x, oB.x, fma(W01.y, oB.y, aB));
-        bB = fma(W23.x, oB.x, fma(W23.y, oB.y, bB));
+        acc(s, W01.x, W01.y, W23.x, W23.y);
     }
 }
 
-// grid = min(ntiles, resident CTAs), block = 16 * P threads (P even),
-// dynamic smem = 20 * blockDim.x * 16 (staging) + 2 * 2 * P * 16 * 16 (forward, backward exchange slots).
-template <bool DIAG>
-__global__ void __launch_bounds__(16 * LINE_MAX_P, 1) k_rhs_sweep_y_line(const __grid_constant__ LineParams prm,
-                                                                        const double *__restrict__ C, double *__restrict__ w,
-                                                                        double *__restrict__ partials)
+// NC = N at compile time (row offsets become immediates).
+// grid = min(ntiles, resident CTAs), block = NC threads (= 16 threads per chunk, P = NC / 16 even),
+// dynamic smem = 20 * NC * 16 (staging) + 2 * 2 * P * 16 * 16 (forward, backward exchange slots).
+// NB: neighbour-warp synchronisation (needs K <= 2) instead of CTA barriers; DIAG kernels use barriers.
+template <int NC, bool DIAG, bool NB>
+__global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_y_line(const __grid_constant__ LineParams prm,
+                                                                                   const double *__restrict__ C,
+                                                                                   double *__restrict__ w,
+                                                                                   double *__restrict__ partials)
 {
-    constexpr int LC = LINE_LC, NR = LC + 4;
+    constexpr int LC = LINE_LC, NR = LC + 4, N = NC, NT = NC, P = NC / LC;
+    constexpr size_t n2 = (size_t)N * N;
     extern __shared__ double2 sm2[];
     __shared__ double red[16][3];
-    const int tid = threadIdx.x, NT = blockDim.x, li = tid & 15, c = tid >> 4;
-    const int N = prm.N, P = prm.P, strips = prm.strips, ntiles = prm.ntiles;
+    __shared__ unsigned flagF[16], flagB[16];
+    static_assert(!(DIAG && NB), "the sampling kernels synchronise with CTA barriers");
+    constexpr int NW = NC / 32;
+    const int tid = threadIdx.x, li = tid & 15, c = tid >> 4, wid = tid >> 5;
+    const int strips = prm.strips, ntiles = prm.ntiles;
+    if (NB) {
+        if (tid < 16) { flagF[tid] = 0; flagB[tid] = 0; }
+        __syncthreads();
+    }
+    unsigned seq = 0;
     const int y0 = c * LC;
-    const size_t n2 = (size_t)N * N;
     const bool lane_ok = li >= 1 && li < 15;
 
     double2 *stage = sm2 + tid;                                   // row j of this thread: stage[j * NT]
     double2 *slotF = sm2 + (size_t)NR * NT, *slotB = slotF + 2 * P * 16;
 
-    // C rows y0-2 .. y0+LC+1 of this thread's column pair; only the two halo rows on either end can wrap
-    auto issue = [&](int tile) {
+    // C rows y0-2 .. y0+LC+1 of this thread's column pair; only the two halo rows on either end wrap
+    auto tile_base = [&](int tile) {
         const int strip = tile % strips, m = tile / strips;
         int gx = strip * LINE_VALID - 2 + 2 * li;
         if (gx < 0) gx += N;
-        while (gx >= N) gx -= N;
-        const double *p = C + (size_t)m * n2 + gx + (ptrdiff_t)(y0 - 2) * N;
-        const double *plo = (c == 0) ? p + n2 : p;
-        const double *phi = (c == P - 1) ? p - n2 : p;
-#pragma unroll
-        for (int j = 0; j < NR; ++j) {
-            const double *q = (j < 2) ? plo : ((j >= LC + 2) ? phi : p);
-            line_cp_async16(stage + j * NT, q + (ptrdiff_t)j * N);
-        }
-        line_cp_async_commit();
+        if (gx >= N) gx -= N;
+        return C + (size_t)m * n2 + gx + (ptrdiff_t)(y0 - 2) * N;
+    };
+    auto load_row = [&](const double *p, int j) {     // j is a compile-time constant after unrolling
+        const double *q = p + (ptrdiff_t)j * N;
+        if (j < 2 && c == 0) q += n2;
+        if (j >= LC + 2 && c == P - 1) q -= n2;
+        line_cp_async16(stage + j * NT, q);
     };
 
     int tile = blockIdx.x;
-    if (tile < ntiles) issue(tile);
+    if (tile < ntiles) {
+        const double *p = tile_base(tile);
+#pragma unroll
+        for (int j = 0; j < NR; ++j) load_row(p, j);
+        line_cp_async_commit();
+    }
     const double np = prm.np, nq = prm.nq, mgam = prm.mgam, k1 = prm.k1;
 
     for (; tile < ntiles; tile += gridDim.x) {
         const int strip = tile % strips, m = tile / strips;
         const int X = strip * LINE_VALID;
         const bool valid = lane_ok && (X + 2 * (li - 1)) < N;
+        const bool more = tile + (int)gridDim.x < ntiles;
+        const double *pn = tile_base(more ? tile + gridDim.x : tile);
         line_cp_async_wait_all();          // a thread reads back only what it staged itself: no barrier needed
 
         double vA[LC], vB[LC];
@@ -138,6 +180,9 @@ __global__ void __launch_bounds__(16 * LINE_MAX_P, 1) k_rhs_sweep_y_line(const _
 #pragma unroll
             for (int k = 0; k < LC; ++k) {
                 const double2 cn = stage[(k + 4) * NT];
+                // staging row k was consumed at least four rows ago: refill it with the NEXT tile's row k,
+                // so the next tile's loads are in flight for a whole tile period
+                if (more) load_row(pn, k);
                 const double2 mu_c = mu_row(c0, c1, cn, k + 1 < LC);   // staged row k + 3
                 const double rA = fma(-4.0, mu_b.x, (ml + mu_b.y) + (mu_a.x + mu_c.x));
                 const double rB = fma(-4.0, mu_b.y, (mu_b.x + mr) + (mu_a.y + mu_c.y));
@@ -153,8 +198,11 @@ __global__ void __launch_bounds__(16 * LINE_MAX_P, 1) k_rhs_sweep_y_line(const _
                 if (k + 1 < LC) { ml = hshfl_up(mu_b.y); mr = hshfl_down(mu_b.x); }
             }
         }
-        // this thread's staging slots are consumed: put the next tile's loads in flight
-        if (tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x);
+        if (more) {
+#pragma unroll
+            for (int j = LC; j < NR; ++j) load_row(pn, j);
+        }
+        line_cp_async_commit();
 
         if (DIAG) {
             // deterministic block sum: warp shuffle, then warps in fixed order
@@ -173,10 +221,18 @@ __global__ void __launch_bounds__(16 * LINE_MAX_P, 1) k_rhs_sweep_y_line(const _
         // ---- forward closure
         slotF[c * 16 + li] = make_double2(vA[LC - 1], vA[LC - 2]);
         slotF[(P + c) * 16 + li] = make_double2(vB[LC - 1], vB[LC - 2]);
-        __syncthreads();
+        ++seq;
+        if (NB) {
+            __syncwarp();
+            if ((tid & 31) == 0) flag_release(&flagF[wid], seq);
+            flag_wait(&flagF[(wid + NW - 1) % NW], seq);
+            __syncwarp();
+        } else {
+            __syncthreads();
+        }
         {
             double aA, bA, aB, bB;
-            line_state_in(prm, slotF, c, li, +1, aA, bA, aB, bB);
+            line_state_in<P>(prm, slotF, c, li, +1, aA, bA, aB, bB);
 #pragma unroll
             for (int k = 0; k < LC; ++k) {
                 vA[k] = fma(prm.alpha[k], aA, fma(prm.beta[k], bA, vA[k]));
@@ -193,13 +249,20 @@ __global__ void __launch_bounds__(16 * LINE_MAX_P, 1) k_rhs_sweep_y_line(const _
         }
         slotB[c * 16 + li] = make_double2(vA[0], vA[1]);
         slotB[(P + c) * 16 + li] = make_double2(vB[0], vB[1]);
-        __syncthreads();      // also orders this tile's slotF reads before the next tile's slotF writes
+        if (NB) {
+            __syncwarp();
+            if ((tid & 31) == 0) flag_release(&flagB[wid], seq);
+            flag_wait(&flagB[(wid + 1) % NW], seq);
+            __syncwarp();
+        } else {
+            __syncthreads();  // also orders this tile's slotF reads before the next tile's slotF writes
+        }
         {
             double aA, bA, aB, bB;
-            line_state_in(prm, slotB, c, li, -1, aA, bA, aB, bB);
+            line_state_in<P>(prm, slotB, c, li, -1, aA, bA, aB, bB);
             if (valid) {
                 const double sc = prm.scale;
-                int gx = X - 2 + 2 * li;                            // valid lanes: 0 <= gx < N
+                const int gx = X - 2 + 2 * li;                      // valid lanes: 0 <= gx < N
                 double2 *wm = reinterpret_cast<double2 *>(w + (size_t)m * n2 + (size_t)y0 * N + gx);
 #pragma unroll
                 for (int k = 0; k < LC; ++k) {
@@ -210,7 +273,8 @@ __global__ void __launch_bounds__(16 * LINE_MAX_P, 1) k_rhs_sweep_y_line(const _
                 }
             }
         }
-        // slotB reads of this tile are ordered before the next tile's slotB writes by the next
-        // tile's first __syncthreads
+        // barrier kernels: slotB reads of this tile are ordered before the next tile's slotB writes by
+        // the next tile's first __syncthreads.  NB kernels: a warp rewrites a slot only after the
+        // neighbour that reads it has published a later sequence number.
     }
 }

@@ -216,11 +216,11 @@ def test_generic_paths_end_to_end(B, oracle):
         assert_series_close(s, so)
 
 
-@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 176, 256, 352, 512, 592, 1024])
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 176, 256, 352, 384, 512, 592, 1024])
 @pytest.mark.parametrize("gamma,dt", [(1.0, 0.01), (66.4, 7.97)])
 def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     """Every 2D step variant against the oracle: the line-fused step (RHS + y-sweep with whole lines
-    in one persistent CTA, N % 32 == 0 and N <= 512; ragged last column strip, more tiles than
+    in one persistent CTA, N in {32, 64, 96, 128, 192, 256, 384, 512}; ragged last column strip, more tiles than
     resident CTAs at M = 40), the cluster-fused step (cluster sizes 1..8) and the three-pass step.
     N = 592 (37 chunks per line) has no legal split and must fall back to three passes by itself."""
     M = 2 if N <= 256 else 1
@@ -232,9 +232,9 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     cs, line, mode = B.ch_get_option(e.ctx, "fused"), B.ch_get_option(e.ctx, "line"), B.ch_get_option(e.ctx, "fuse_mode")
     e.close()
     assert (cs == 0) == (N == 592)
-    assert (line != 0) == (N % 32 == 0 and N <= 512)
+    assert (line != 0) == (N in (32, 64, 96, 128, 192, 256, 384, 512))
     assert mode == (3 if line else (2 if cs else 0))
-    variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}] if line else [])
+    variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}] if line else [])
     for opts in variants:
         C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options=opts)
         assert np.abs(C - Co).max() <= tol, (N, opts)
