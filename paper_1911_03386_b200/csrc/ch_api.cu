@@ -543,13 +543,13 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
 {
     LineParams p;
     p.np = c->fac.np; p.nq = c->fac.nq;
-    p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0; p.scale = c->rscale;
+    p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0;
     memcpy(p.alpha, c->fac.alpha, sizeof(p.alpha));
     memcpy(p.beta, c->fac.beta, sizeof(p.beta));
     memcpy(p.W0, c->fac.W[0], sizeof(p.W0));
     memcpy(p.W1, c->fac.W[1], sizeof(p.W1));
     p.W = c->dW; p.K = c->fac.K;
-    p.strips = c->l_strips; p.ntiles = c->l_strips * c->M; p.write = write ? 1 : 0;
+    p.ntiles = c->l_strips * c->M; p.write = write ? 1 : 0;
     const int grid = p.ntiles < c->l_resident ? p.ntiles : c->l_resident;
     const size_t smem = line_smem(c->N);
     const bool nb = p.K <= 2 && c->opt_linesync != 1;     // neighbour-warp synchronisation instead of CTA barriers
@@ -590,7 +590,8 @@ static void launch_sweep_x_update(ch_ctx *c)
 {
     ProfScope ps(c, KIND_SWEEP_X_UPDATE);
     SweepParams prm;
-    fill_params(c, prm, 1.0);
+    // the line kernel leaves the RHS scale dt / c0^2 to this kernel's final fused multiply-add
+    fill_params(c, prm, fuse_mode(c) == 3 ? c->rscale : 1.0);
     const int N = c->N, P = c->fac.P;
     const long long total_lines = (long long)c->M * N;
     int threads = 256;

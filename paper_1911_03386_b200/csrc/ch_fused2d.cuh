@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(512) k_rhs_sweep_y(const __grid_constant__ Swe
 }
 
 // ------------------------------------------------------------------------------------
-// k_sweep_x_update: C += A_x^-1 w on contiguous lines.  CTA = LPB consecutive lines; both the w
+// k_sweep_x_update: C += oscale * A_x^-1 w on contiguous lines.  CTA = LPB consecutive lines; both the w
 // lines and the matching C lines are brought in with cp.async (16-byte, L2 only); w lands in the
 // 16-byte-granule XOR swizzle of k_sweep_contig so the chunk phase (LDS.128 at a lane stride of
 // LC*8 bytes) is bank-conflict free.  block = LPB * P threads,
@@ -279,6 +279,6 @@ __global__ void k_sweep_x_update(const __grid_constant__ SweepParams prm, const 
     __syncthreads();
     for (int g = t; g < G; g += nthreads) {
         const double2 x = sl[swz<LC>(g)], cc = sC[g];
-        gC[g] = make_double2(cc.x + x.x, cc.y + x.y);
+        gC[g] = make_double2(fma(prm.oscale, x.x, cc.x), fma(prm.oscale, x.y, cc.y));
     }
 }

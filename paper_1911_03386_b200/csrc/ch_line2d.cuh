@@ -1,7 +1,7 @@
 // ch_line2d.cuh -- fused RHS + y-sweep of the 2D step for lines that fit one CTA (N <= 512).
 // DESIGN.md section 5.
 //
-//   k_rhs_sweep_y_line   w = A_y^-1 (scale * Lap_h mu(C))                     P:29-30, include/ch.h
+//   k_rhs_sweep_y_line   w = A_y^-1 Lap_h mu(C)   (scale applied by k_sweep_x_update)                   P:29-30, include/ch.h
 //                        (+ fused F, Fdot, mass partials on sampling steps)
 //
 // A persistent CTA owns whole columns: tile = one column strip (28 produced columns + a halo of 2 on
@@ -26,11 +26,11 @@
 
 struct LineParams {
     double np, nq;                  // recurrence  z_i = b_i + np z_{i-1} + nq z_{i-2}
-    double gamma, mgam, k1, scale;  // mu = c (c^2 + k1) - gamma * (sum of the 4 neighbours), k1 = 4 gamma - 1
+    double gamma, mgam, k1;         // mu = c (c^2 + k1) - gamma * (sum of the 4 neighbours), k1 = 4 gamma - 1
     double alpha[LINE_LC], beta[LINE_LC];
     double W0[4], W1[4];            // first two closure matrices (all of them when K <= 2)
     const double *W;                // device [K][4] (ch_factor.h)
-    int K, strips, ntiles, write;
+    int K, ntiles, write;
 };
 
 __device__ __forceinline__ void line_cp_async16(void *smem_dst, const void *gsrc)
@@ -62,12 +62,17 @@ __device__ __forceinline__ void flag_wait(const unsigned *flag, unsigned seq)
     } while (v < seq);
 }
 
+// keeps the compiler from carrying values derived from x across the long tile body in registers:
+// what is needed again at the end of a tile is recomputed there from an opaque copy
+__device__ __forceinline__ int opaque(int x) { asm volatile("" : "+r"(x)); return x; }
+
 // states entering chunk c (both columns of the lane) from the K chunks before it (dir = +1) or after
 // it (dir = -1); slots are [column A|B][chunk][16 lanes] pairs (value next to the boundary, one further in)
 template <int P>
-__device__ __forceinline__ void line_state_in(const LineParams &prm, const double2 *slots, int c, int li, int dir,
+__device__ __forceinline__ void line_state_in(const LineParams &prm, const double2 *slots, int tid, int dir,
                                               double &aA, double &bA, double &aB, double &bB)
 {
+    const int c = tid >> 4, li = tid & 15;
     aA = bA = aB = bB = 0.0;
     auto acc = [&](int s, double w0, double w1, double w2, double w3) {
         const double2 oA = slots[s * 16 + li], oB = slots[(P + s) * 16 + li];
@@ -109,7 +114,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
     static_assert(!(DIAG && NB), "the sampling kernels synchronise with CTA barriers");
     constexpr int NW = NC / 32;
     const int tid = threadIdx.x, li = tid & 15, c = tid >> 4, wid = tid >> 5;
-    const int strips = prm.strips, ntiles = prm.ntiles;
+    constexpr int strips = (NC + LINE_VALID - 1) / LINE_VALID;
+    const int ntiles = prm.ntiles;
     if (NB) {
         if (tid < 16) { flagF[tid] = 0; flagB[tid] = 0; }
         __syncthreads();
@@ -147,8 +153,7 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
 
     for (; tile < ntiles; tile += gridDim.x) {
         const int strip = tile % strips, m = tile / strips;
-        const int X = strip * LINE_VALID;
-        const bool valid = lane_ok && (X + 2 * (li - 1)) < N;
+        const bool valid = lane_ok && (strip * LINE_VALID + 2 * (li - 1)) < N;     // used by the DIAG sums only
         const bool more = tile + (int)gridDim.x < ntiles;
         const double *pn = tile_base(more ? tile + gridDim.x : tile);
         line_cp_async_wait_all();          // a thread reads back only what it staged itself: no barrier needed
@@ -219,8 +224,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
 
         // ---- forward closure
-        slotF[c * 16 + li] = make_double2(vA[LC - 1], vA[LC - 2]);
-        slotF[(P + c) * 16 + li] = make_double2(vB[LC - 1], vB[LC - 2]);
+        slotF[tid] = make_double2(vA[LC - 1], vA[LC - 2]);              // [column A|B][chunk][lane]: c * 16 + li == tid
+        slotF[NT + tid] = make_double2(vB[LC - 1], vB[LC - 2]);
         ++seq;
         if (NB) {
             __syncwarp();
@@ -232,7 +237,7 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
         {
             double aA, bA, aB, bB;
-            line_state_in<P>(prm, slotF, c, li, +1, aA, bA, aB, bB);
+            line_state_in<P>(prm, slotF, tid, +1, aA, bA, aB, bB);
 #pragma unroll
             for (int k = 0; k < LC; ++k) {
                 vA[k] = fma(prm.alpha[k], aA, fma(prm.beta[k], bA, vA[k]));
@@ -247,8 +252,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
             vA[k] = fma(np, vA[k + 1], fma(nq, vA[k + 2], vA[k]));
             vB[k] = fma(np, vB[k + 1], fma(nq, vB[k + 2], vB[k]));
         }
-        slotB[c * 16 + li] = make_double2(vA[0], vA[1]);
-        slotB[(P + c) * 16 + li] = make_double2(vB[0], vB[1]);
+        slotB[tid] = make_double2(vA[0], vA[1]);
+        slotB[NT + tid] = make_double2(vB[0], vB[1]);
         if (NB) {
             __syncwarp();
             if ((tid & 31) == 0) flag_release(&flagB[wid], seq);
@@ -259,16 +264,18 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
         {
             double aA, bA, aB, bB;
-            line_state_in<P>(prm, slotB, c, li, -1, aA, bA, aB, bB);
-            if (valid) {
-                const double sc = prm.scale;
-                const int gx = X - 2 + 2 * li;                      // valid lanes: 0 <= gx < N
-                double2 *wm = reinterpret_cast<double2 *>(w + (size_t)m * n2 + (size_t)y0 * N + gx);
+            line_state_in<P>(prm, slotB, tid, -1, aA, bA, aB, bB);
+            // where this thread's results go, recomputed from the tile and thread index
+            const int t2 = opaque(tile), tid2 = opaque(tid);
+            const int strip2 = t2 % strips, m2 = t2 / strips, li2 = tid2 & 15;
+            const int gx = strip2 * LINE_VALID - 2 + 2 * li2;
+            if (li2 >= 1 && li2 < 15 && gx < N) {                   // producing lanes: 0 <= gx < N
+                double2 *wm = reinterpret_cast<double2 *>(w + (size_t)m2 * n2 + (size_t)(tid2 >> 4) * (LC * N) + gx);
 #pragma unroll
                 for (int k = 0; k < LC; ++k) {
                     double2 o;
-                    o.x = sc * fma(prm.alpha[LC - 1 - k], aA, fma(prm.beta[LC - 1 - k], bA, vA[k]));
-                    o.y = sc * fma(prm.alpha[LC - 1 - k], aB, fma(prm.beta[LC - 1 - k], bB, vB[k]));
+                    o.x = fma(prm.alpha[LC - 1 - k], aA, fma(prm.beta[LC - 1 - k], bA, vA[k]));
+                    o.y = fma(prm.alpha[LC - 1 - k], aB, fma(prm.beta[LC - 1 - k], bB, vB[k]));
                     wm[(size_t)k * (N / 2)] = o;
                 }
             }
