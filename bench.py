@@ -36,7 +36,12 @@ ALGO_BYTES = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, kernel); None until captured.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r01_v6_ncu_full_cfg3.md (k_sweep_x_update<16>: 536.9 MB read + 215.8 MB written; the rest of
+    # the 268 MB write-back was still in L2 when the launch ended)
+    ("cfg3", "sweep_x_update"): 752.7e6,
+    ("cfg3", "rhs_sweep_y"): 487.7e6,
+}
 
 
 def workload_desc(name):
@@ -220,15 +225,22 @@ def run_ours(args):
             kernels[kind] = {"launches": cnt, "avg_ms": avg, "algo_bytes_per_update": ALGO_BYTES[D][kind],
                              "achieved_gbs": gbs, "frac": gbs / peak}
     total_kernel_ms = sum(ms for ms, _ in prof.values())
+    # bytes one step must move in the pass structure that ran: fused 2D step 16 + 24 = 40 B per update
+    # (DESIGN.md section 5), three-pass 2D 56 B, four-pass 3D 72 B
+    fused = "sweep_x_update" in kernels
+    step_bytes = 40 if fused else (56 if D == 2 else 72)
+    model_bytes = 56 if D == 2 else 72
     main_kinds = {k: v for k, v in kernels.items() if not k.endswith("_diag")} or kernels
     dom = max(main_kinds, key=lambda k: main_kinds[k]["avg_ms"] * main_kinds[k]["launches"])
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES.get((name, dom)),
                 "peak_source": peak_src, "share_of_step": kernels[dom]["avg_ms"] * kernels[dom]["launches"] / total_kernel_ms,
-                "step_algo_bytes_per_update": 56 if D == 2 else 72,
-                "step_achieved_gbs": value / world * (56 if D == 2 else 72) / 1e9,
-                "step_frac": value / world * (56 if D == 2 else 72) / 1e9 / peak,
-                "step_frac_of_8TBs_nominal": value / world * (56 if D == 2 else 72) / 1e9 / 8000.0}
+                "step_algo_bytes_per_update": step_bytes,
+                "step_achieved_gbs": value / world * step_bytes / 1e9,
+                "step_frac": value / world * step_bytes / 1e9 / peak,
+                "step_frac_of_8TBs_nominal": value / world * step_bytes / 1e9 / 8000.0,
+                "unfused_model_bytes_per_update": model_bytes,
+                "unfused_model_frac": value / world * model_bytes / 1e9 / peak}
 
     # ---- end-to-end leg: the user's job through the C ABI with HOST buffers (pinned):
     # ch_set_state(host) -> ch_step(K) with the series -> series D2H + ch_energy(host) + ch_get_state(host)
