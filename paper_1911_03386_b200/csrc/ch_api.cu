@@ -12,6 +12,7 @@
 #include "ch_kernels.cuh"
 #include "ch_fused2d.cuh"
 #include "ch_line2d.cuh"
+#include "ch_rhs3d_stream.cuh"
 
 enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z,
        KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_COUNT };
@@ -54,6 +55,10 @@ struct ch_ctx {
     // fused 2D step (ch_fused2d.cuh)
     bool fused_ok;
     int f_CPB, f_CS, f_strips;   // chunks per CTA, CTAs per cluster, column strips per member
+    // streaming 3D RHS (ch_rhs3d_stream.cuh)
+    bool r3_ok;
+    int r3_parts, r3_resident;   // partials per member, CTAs resident on the device
+    int opt_rhs3;                // 0 auto (streaming kernel when available), 1 tile kernel
     // fused 2D step, whole line in one CTA (ch_line2d.cuh)
     bool line_ok;
     int l_strips, l_resident;    // column strips per member, CTAs resident on the device
@@ -71,6 +76,8 @@ static int fuse_mode(const ch_ctx *c)
     if (c->opt_fuse == 3) return c->line_ok ? 3 : 0;
     return c->line_ok ? 3 : (c->fused_ok ? 2 : 0);
 }
+
+static bool use_rhs3_stream(const ch_ctx *c) { return c->r3_ok && c->opt_rhs3 != 1; }
 
 // Brackets one kernel launch with CUDA events on the context's stream when profiling is on.
 struct ProfScope {
@@ -146,6 +153,13 @@ static bool line_geometry(int N, int D, int *strips)
     return true;
 }
 
+static bool rhs3_stream_geometry(int N, int D, int *parts)
+{
+    if (D != 3 || (N != 64 && N != 128)) return false;
+    *parts = ((N + R3_VALID - 1) / R3_VALID) * (N / R3_ZR);
+    return true;
+}
+
 static size_t line_smem(int N)
 {
     const int P = N / LINE_LC;
@@ -157,6 +171,7 @@ static int max_parts(int N, int D)
     int n = rhs_parts(N, D), cpb, cs, st;
     if (fused_geometry(N, D, &cpb, &cs, &st) && st * cs > n) n = st * cs;
     if (line_geometry(N, D, &st) && st > n) n = st;
+    if (rhs3_stream_geometry(N, D, &st) && st > n) n = st;
     return n;
 }
 
@@ -222,6 +237,26 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->launches = 0; c->profiling = false;
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
+    c->r3_parts = 0; c->r3_resident = 0; c->opt_rhs3 = 0;
+    c->r3_ok = rhs3_stream_geometry(N, D, &c->r3_parts);
+    if (c->r3_ok) {
+        const int smem = (int)rhs3_stream_smem(N);
+        int per_sm = 0, dev = 0, sms = 0;
+        cudaError_t e = cudaErrorInvalidValue;
+#define X(NC)                                                                                                        \
+        if (N == NC) {                                                                                               \
+            e = cudaFuncSetAttribute(k_rhs3d_stream<NC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);  \
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs3d_stream<NC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_rhs3d_stream<NC, false>, 4 * NC, smem); \
+        }
+        X(64) X(128)
+#undef X
+        if (e == cudaSuccess) e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || per_sm < 1 || sms < 1) c->r3_ok = false;
+        else c->r3_resident = per_sm * sms;
+        cudaGetLastError();
+    }
     c->l_strips = 0; c->l_resident = 0;
     c->line_ok = line_geometry(N, D, &c->l_strips);
     if (c->chunked) {
@@ -393,6 +428,11 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_sweep = value;
         return CH_OK;
     }
+    if (!strcmp(key, "rhs3")) {
+        if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: rhs3 must be 0 (auto) or 1 (tile kernel)");
+        ctx->opt_rhs3 = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "linesync")) {
         if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: linesync must be 0 (auto) or 1 (CTA barriers)");
         ctx->opt_linesync = value;
@@ -416,6 +456,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
     if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
     if (!strcmp(key, "fused")) { *value = ctx->fused_ok ? ctx->f_CS : 0; return CH_OK; }
+    if (!strcmp(key, "rhs3_stream")) { *value = use_rhs3_stream(ctx) ? ctx->r3_resident : 0; return CH_OK; }
     if (!strcmp(key, "line")) { *value = ctx->line_ok ? ctx->l_resident : 0; return CH_OK; }
     if (!strcmp(key, "fuse_mode")) { *value = fuse_mode(ctx); return CH_OK; }
     return CH_EINVAL;
@@ -424,10 +465,23 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
 // ---------------------------------------------------------------------------------------
 // launches
 // ---------------------------------------------------------------------------------------
+// partials per member the RHS kernel in use writes on the three-/four-pass path
+static int rhs_parts_in_use(const ch_ctx *c) { return use_rhs3_stream(c) ? c->r3_parts : c->nparts; }
+
 template <bool DIAG, bool WRITE>
 static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
 {
     ProfScope ps(c, DIAG ? KIND_RHS_DIAG : KIND_RHS);
+    if (use_rhs3_stream(c)) {
+        Rhs3Params p;
+        p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 6.0 * c->gamma - 1.0; p.scale = scale;
+        p.nunits = c->r3_parts * c->M; p.write = WRITE ? 1 : 0;
+        const int grid = p.nunits < c->r3_resident ? p.nunits : c->r3_resident;
+        const size_t smem = rhs3_stream_smem(c->N);
+        if (c->N == 64) k_rhs3d_stream<64, DIAG><<<grid, 256, smem, c->stream>>>(p, C, r, c->partials);
+        else k_rhs3d_stream<128, DIAG><<<grid, 512, smem, c->stream>>>(p, C, r, c->partials);
+        return;
+    }
     if (c->D == 2) {
         dim3 grid(c->nparts, c->M);
         if (c->pow2) k_rhs2d<DIAG, WRITE, true><<<grid, 256, 0, c->stream>>>(C, r, c->partials, c->N, c->gamma, scale, c->rhs_tiles_x);
@@ -583,7 +637,7 @@ static int launch_diag_only(ch_ctx *c)
 {
     if (use_fused(c)) { launch_rhs_sweep_y(c, true, false); return fused_parts(c); }
     launch_rhs(c, c->C, c->w, c->rscale, true, false);
-    return c->nparts;
+    return rhs_parts_in_use(c);
 }
 
 static void launch_sweep_x_update(ch_ctx *c)
@@ -633,7 +687,7 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
         else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
         if (sample) {
             launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
-                          fused ? fused_parts(ctx) : ctx->nparts);
+                          fused ? fused_parts(ctx) : rhs_parts_in_use(ctx));
             ctx->cursor++; ctx->last_sampled = ctx->n;
         }
         if (fused) launch_sweep_x_update(ctx);

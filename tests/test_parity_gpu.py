@@ -51,7 +51,7 @@ def run_gpu(B, C0, gamma, dt, nsteps, stride, options=None, t0=0.0):
 # ------------------------------------------------------------------ per kernel
 @pytest.mark.parametrize("N,D,M,gamma,dt", [
     (64, 2, 3, 1.0, 0.01), (512, 2, 2, 1.0, 0.01), (24, 2, 2, 1.0, 0.01), (8, 2, 1, 1.0, 0.01),
-    (100, 2, 1, 0.5, 0.02), (32, 3, 2, 1.0, 0.01), (128, 3, 1, 1.0, 0.01), (20, 3, 1, 1.0, 0.01), (8, 3, 1, 2.0, 0.01),
+    (100, 2, 1, 0.5, 0.02), (32, 3, 2, 1.0, 0.01), (128, 3, 1, 1.0, 0.01), (64, 3, 3, 0.7, 0.02), (20, 3, 1, 1.0, 0.01), (8, 3, 1, 2.0, 0.01),
 ])
 def test_rhs_kernel(B, oracle, N, D, M, gamma, dt):
     C0 = inputs.initial_state(range(50, 50 + M), N, D, -0.2, 0.5)
@@ -84,7 +84,7 @@ def test_sweep_kernels(B, oracle, N, D, M, sigma):
 
 
 def test_energy_kernel(B, oracle):
-    for N, D in [(64, 2), (512, 2), (24, 2), (32, 3), (20, 3)]:
+    for N, D in [(64, 2), (512, 2), (24, 2), (32, 3), (20, 3), (64, 3), (128, 3)]:
         C0 = inputs.initial_state([1, 2], N, D, [0.0, -0.4], 0.3)
         e = B.Ensemble(2, N, D, 1.3, 0.01)
         e.set_state(C0)
@@ -154,6 +154,23 @@ def test_cfg4_3d_member_subset(B, oracle):
     C, s = run_gpu(B, C0, c["gamma"], c["dt"], 100, c["stride"])
     sub = [0, 15]
     Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 100, c["stride"])
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
+
+
+def test_3d_streaming_and_tile_rhs(B, oracle):
+    """64^3 (the z-marching RHS kernel, several work units per CTA at M = 12) against the oracle and
+    against the tile RHS kernel on the same data."""
+    C0 = inputs.initial_state(range(3100, 3112), 64, 3, [0.0, -0.4] * 6, 0.05)
+    e = B.Ensemble(12, 64, 3, 1.0, 0.01)
+    assert B.ch_get_option(e.ctx, "rhs3_stream") > 0
+    e.close()
+    C, s = run_gpu(B, C0, 1.0, 0.01, 60, 20)
+    Ct, st = run_gpu(B, C0, 1.0, 0.01, 60, 20, options={"rhs3": 1})
+    assert np.abs(C - Ct).max() <= 1e-13
+    assert_series_close(s, st, 1e-12)
+    sub = [0, 5, 11]
+    Co, so = oracle.run(C0[sub], 1.0, 0.01, 60, 20)
     assert np.abs(C[sub] - Co).max() <= FIELD_TOL
     assert_series_close(s[:, sub], so)
 
