@@ -276,6 +276,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     cudaFuncSetAttribute(k_rhs3d<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
     cudaFuncSetAttribute(k_rhs3d<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
     cudaFuncSetAttribute(k_rhs3d<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHS3_SMEM);
+    cudaFuncSetAttribute(k_sweep_pcr_x, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     cudaFuncSetAttribute(k_sweep_contig<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
     cudaFuncSetAttribute(k_sweep_contig<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
     cudaFuncSetAttribute(k_sweep_contig<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
@@ -423,7 +424,8 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
 {
     if (!ctx || !key) return CH_EINVAL;
     if (!strcmp(key, "sweep")) {
-        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: sweep must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(ctx, CH_EINVAL, "ch_set_option: sweep must be 0 (auto), 1 (generic), 2 (chunked LU) or 3 (PCR x-sweep)");
+        if (value == 3 && !(ctx->pow2 && ctx->N <= 4096)) return fail(ctx, CH_EINVAL, "ch_set_option: the PCR sweep needs N a power of two <= 4096");
         if (value == 2 && !ctx->chunked) return fail(ctx, CH_EINVAL, "ch_set_option: chunked sweeps need N % 16 == 0");
         ctx->opt_sweep = value;
         return CH_OK;
@@ -521,6 +523,25 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
     const size_t n2 = (size_t)N * N, n3 = n2 * N;
     const bool chunked = c->chunked && c->opt_sweep != 1;
     ProfScope ps(c, KIND_SWEEP_X + axis);
+    if (c->opt_sweep == 3 && axis == 0 && !update) {
+        // parallel cyclic reduction (measured alternative); level tables in long double
+        PcrParams p;
+        long double a = c->fac.sigma / (1 + 6 * (long double)c->fac.sigma), b = -4 * a;
+        const long double norm = 1 / (1 + 6 * (long double)c->fac.sigma);    // the initial division by the diagonal
+        int L = 0;
+        for (int st = 1; st < N && L < CH_PCR_MAX_LEVELS; st <<= 1, ++L) {
+            if (fabsl(a) < 1e-22L && fabsl(b) < 1e-22L) break;
+            const long double cp = 1 + 2 * a * a - 2 * b * b;
+            p.A[L] = (double)(a / cp); p.B[L] = (double)(-b / cp); p.Cc[L] = (double)(1 / cp);
+            const long double a2 = a * a / cp, b2 = (2 * a - b * b) / cp;
+            a = a2; b = b2;
+        }
+        p.levels = L;
+        p.final_scale = (double)(norm / (1 + 2 * a + 2 * b)) * c->fac.c0 * (scale ? oscale : 1.0);
+        const long long total_lines = (long long)M * (D == 3 ? n2 : (size_t)N);
+        k_sweep_pcr_x<<<(unsigned)total_lines, 256, (size_t)2 * N * 8, c->stream>>>(p, w, N);
+        return;
+    }
     if (!chunked) {
         long long n_lines = (long long)M * (D == 3 ? n2 : (size_t)N);
         int n_inner; size_t os, is, ls;

@@ -83,6 +83,19 @@ def test_sweep_kernels(B, oracle, N, D, M, sigma):
     e.close()
 
 
+@pytest.mark.parametrize("N,D,M", [(8, 2, 2), (64, 2, 3), (1024, 2, 1), (2048, 2, 1), (4096, 2, 1), (32, 3, 1)])
+@pytest.mark.parametrize("sigma", [0.01, 1.0, 529.0])
+def test_pcr_x_sweep(B, oracle, N, D, M, sigma):
+    """The parallel-cyclic-reduction x-sweep (option sweep = 3; the north star's measured alternative
+    for N >= 1024) against the oracle's banded solve, truncated (sigma = 0.01) and full depth."""
+    rng = np.random.default_rng(N + D)
+    w = rng.standard_normal((M,) + (N,) * D)
+    e = B.Ensemble(M, N, D, sigma / 0.5, 0.5, options={"sweep": 3})
+    got, ref = e.sweep(w, 0), oracle.sweep(w, sigma, 0)
+    e.close()
+    assert np.abs(got - ref).max() <= 1e-14 * (1 + 16 * sigma) * np.abs(ref).max()
+
+
 def test_energy_kernel(B, oracle):
     for N, D in [(64, 2), (512, 2), (24, 2), (32, 3), (20, 3), (64, 3), (128, 3)]:
         C0 = inputs.initial_state([1, 2], N, D, [0.0, -0.4], 0.3)
