@@ -13,6 +13,7 @@
 #include "ch_fused2d.cuh"
 #include "ch_line2d.cuh"
 #include "ch_rhs3d_stream.cuh"
+#include "ch_cline2d.cuh"
 
 enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z,
        KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_COUNT };
@@ -55,6 +56,10 @@ struct ch_ctx {
     // fused 2D step (ch_fused2d.cuh)
     bool fused_ok;
     int f_CPB, f_CS, f_strips;   // chunks per CTA, CTAs per cluster, column strips per member
+    // fused 2D step, line spread over a cluster of 512-row CTAs (ch_cline2d.cuh); needs K <= 2 at LC = 16
+    bool cline_ok;
+    int cl_CS, cl_strips, cl_resident;   // cluster size, column strips per member, clusters resident on the device
+    ChFactor fac16;                      // factorisation tables at chunk length 16 (c->fac may use 32)
     // streaming 3D RHS (ch_rhs3d_stream.cuh)
     bool r3_ok;
     int r3_parts, r3_resident;   // partials per member, CTAs resident on the device
@@ -68,13 +73,15 @@ struct ch_ctx {
     std::string err;
 };
 
-// which fused 2D step runs: 0 none (three-pass), 2 cluster kernel, 3 line kernel
+// which fused 2D step runs: 0 none (three-pass), 2 st.async cluster kernel, 3 line kernel, 4 cluster line kernel
+// (mode 4 steps with the cluster line kernel and samples with the mode-2 kernel)
 static int fuse_mode(const ch_ctx *c)
 {
     if (c->opt_fuse == 1 || c->opt_sweep == 1) return 0;
     if (c->opt_fuse == 2) return c->fused_ok ? 2 : 0;
     if (c->opt_fuse == 3) return c->line_ok ? 3 : 0;
-    return c->line_ok ? 3 : (c->fused_ok ? 2 : 0);
+    if (c->opt_fuse == 4) return c->cline_ok ? 4 : 0;
+    return c->line_ok ? 3 : (c->cline_ok ? 4 : (c->fused_ok ? 2 : 0));
 }
 
 static bool use_rhs3_stream(const ch_ctx *c) { return c->r3_ok && c->opt_rhs3 != 1; }
@@ -237,6 +244,28 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->launches = 0; c->profiling = false;
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
+    c->cline_ok = false; c->cl_CS = 0; c->cl_strips = 0; c->cl_resident = 0;
+    if (D == 2 && c->fused_ok && (N == 1024 || N == 2048) && ch_factor_build(&c->fac16, N, gamma * dt, LINE_LC) == 0
+        && c->fac16.K <= 2) {
+        c->cl_CS = N / CLINE_NC; c->cl_strips = (N + LINE_VALID - 1) / LINE_VALID;
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = c->cl_CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.gridDim = dim3(c->cl_CS * 64); cfg.blockDim = dim3(CLINE_NC); cfg.dynamicSmemBytes = cline_smem();
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int ncl = 0;
+        cudaError_t e;
+        if (c->cl_CS == 2) {
+            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<2>, &cfg);
+        } else {
+            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<4>, &cfg);
+        }
+        if (e == cudaSuccess && ncl >= 1) { c->cline_ok = true; c->cl_resident = ncl; }
+        cudaGetLastError();
+    }
     c->r3_parts = 0; c->r3_resident = 0; c->opt_rhs3 = 0;
     c->r3_ok = rhs3_stream_geometry(N, D, &c->r3_parts);
     if (c->r3_ok) {
@@ -441,7 +470,8 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         return CH_OK;
     }
     if (!strcmp(key, "fuse")) {
-        if (value < 0 || value > 3) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster) or 3 (line)");
+        if (value < 0 || value > 4) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line) or 4 (cluster line)");
+        if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2, N in {1024, 2048} and a closure truncated to 2 chunks");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
         if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 192, 256, 384, 512}");
         ctx->opt_fuse = value;
@@ -459,6 +489,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
     if (!strcmp(key, "fused")) { *value = ctx->fused_ok ? ctx->f_CS : 0; return CH_OK; }
     if (!strcmp(key, "rhs3_stream")) { *value = use_rhs3_stream(ctx) ? ctx->r3_resident : 0; return CH_OK; }
+    if (!strcmp(key, "cline")) { *value = ctx->cline_ok ? ctx->cl_resident : 0; return CH_OK; }
     if (!strcmp(key, "line")) { *value = ctx->line_ok ? ctx->l_resident : 0; return CH_OK; }
     if (!strcmp(key, "fuse_mode")) { *value = fuse_mode(ctx); return CH_OK; }
     return CH_EINVAL;
@@ -638,18 +669,44 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
 #undef X
 }
 
+static void launch_rhs_sweep_y_cline(ch_ctx *c)
+{
+    LineParams p;
+    const ChFactor &f = c->fac16;
+    p.np = f.np; p.nq = f.nq;
+    p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0;
+    memcpy(p.alpha, f.alpha, sizeof(p.alpha));
+    memcpy(p.beta, f.beta, sizeof(p.beta));
+    memcpy(p.W0, f.W[0], sizeof(p.W0));
+    memcpy(p.W1, f.W[1], sizeof(p.W1));
+    p.W = nullptr; p.K = f.K;
+    p.ntiles = c->cl_strips * c->M; p.write = 1;
+    const int ncl = p.ntiles < c->cl_resident ? p.ntiles : c->cl_resident;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = c->cl_CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.gridDim = dim3(c->cl_CS * ncl); cfg.blockDim = dim3(CLINE_NC); cfg.dynamicSmemBytes = cline_smem();
+    cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = 1;
+    if (c->cl_CS == 2) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<2>, p, (const double *)c->C, c->w);
+    else cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<4>, p, (const double *)c->C, c->w);
+}
+
 // number of F/Fdot/mass partials per member the fused RHS kernel in use writes
 static int fused_parts(const ch_ctx *c) { return fuse_mode(c) == 3 ? c->l_strips : c->f_strips * c->f_CS; }
 
-// diag: also reduce F, Fdot, mass of C^n into the partials; write == false (diag only): no sweep, w untouched
-static void launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
+// diag: also reduce F, Fdot, mass of C^n into the partials; write == false (diag only): no sweep, w untouched.
+// Returns true when w is left WITHOUT the RHS scale dt / c0^2 (k_sweep_x_update then applies it).
+static bool launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
 {
     ProfScope ps(c, diag ? KIND_RHS_SWEEP_Y_DIAG : KIND_RHS_SWEEP_Y);
-    if (fuse_mode(c) == 3) { launch_rhs_sweep_y_line(c, diag, write); return; }
+    if (fuse_mode(c) == 3) { launch_rhs_sweep_y_line(c, diag, write); return true; }
+    if (fuse_mode(c) == 4 && !diag) { launch_rhs_sweep_y_cline(c); return true; }
     SweepParams prm;
     fill_params(c, prm, 1.0);
     if (c->LC == 16) { if (diag) launch_rhs_sweep_y_t<16, true>(c, prm, write); else launch_rhs_sweep_y_t<16, false>(c, prm, 1); }
     else { if (diag) launch_rhs_sweep_y_t<32, true>(c, prm, write); else launch_rhs_sweep_y_t<32, false>(c, prm, 1); }
+    return false;
 }
 
 // F, Fdot, mass partials of the current state with the same kernel (hence the same summation order)
@@ -661,12 +718,12 @@ static int launch_diag_only(ch_ctx *c)
     return rhs_parts_in_use(c);
 }
 
-static void launch_sweep_x_update(ch_ctx *c)
+static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
 {
     ProfScope ps(c, KIND_SWEEP_X_UPDATE);
     SweepParams prm;
-    // the line kernel leaves the RHS scale dt / c0^2 to this kernel's final fused multiply-add
-    fill_params(c, prm, fuse_mode(c) == 3 ? c->rscale : 1.0);
+    // the line kernels leave the RHS scale dt / c0^2 to this kernel's final fused multiply-add
+    fill_params(c, prm, unscaled ? c->rscale : 1.0);
     const int N = c->N, P = c->fac.P;
     const long long total_lines = (long long)c->M * N;
     int threads = 256;
@@ -704,14 +761,15 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
     const bool fused = use_fused(ctx);
     for (int s = 0; s < nsteps; ++s) {
         const bool sample = ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n;
-        if (fused) launch_rhs_sweep_y(ctx, sample, true);
+        bool unscaled = false;
+        if (fused) unscaled = launch_rhs_sweep_y(ctx, sample, true);
         else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
         if (sample) {
             launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
                           fused ? fused_parts(ctx) : rhs_parts_in_use(ctx));
             ctx->cursor++; ctx->last_sampled = ctx->n;
         }
-        if (fused) launch_sweep_x_update(ctx);
+        if (fused) launch_sweep_x_update(ctx, unscaled);
         else for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
         ctx->n++;
     }

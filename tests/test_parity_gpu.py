@@ -260,11 +260,14 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     tol, rtol = (FIELD_TOL, SERIES_RTOL) if gamma == 1.0 else (1e-9, 1e-7)
     e = B.Ensemble(M, N, 2, gamma, dt)
     cs, line, mode = B.ch_get_option(e.ctx, "fused"), B.ch_get_option(e.ctx, "line"), B.ch_get_option(e.ctx, "fuse_mode")
+    cline = B.ch_get_option(e.ctx, "cline")
     e.close()
     assert (cs == 0) == (N == 592)
     assert (line != 0) == (N in (32, 64, 96, 128, 192, 256, 384, 512))
-    assert mode == (3 if line else (2 if cs else 0))
-    variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}] if line else [])
+    assert (cline != 0) == (N == 1024 and gamma == 1.0)        # K <= 2 only: not in the paper regime
+    assert mode == (3 if line else (4 if cline else (2 if cs else 0)))
+    variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}] if line else []) \
+        + ([{"fuse": 4}] if cline else [])
     for opts in variants:
         C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options=opts)
         assert np.abs(C - Co).max() <= tol, (N, opts)
