@@ -51,6 +51,7 @@ struct ch_ctx {
     cudaStream_t stream;
     // options
     int opt_sweep;          // 0 auto, 1 generic, 2 chunked
+    int opt_scan;           // contiguous sweeps: 0 auto (shuffle-scan closure when K > 4), 1 off, 2 always
     int opt_linesync;       // line kernel: 0 auto (neighbour-warp sync when K <= 2), 1 CTA barriers
     int opt_fuse;           // 0 auto (fused 2D step when available), 1 off, 2 cluster kernel, 3 line kernel
     // fused 2D step (ch_fused2d.cuh)
@@ -241,7 +242,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->C = c->w = c->partials = c->eout = nullptr;
     c->has_state = false; c->n = 0; c->t0 = 0.0;
     c->series = nullptr; c->stride = 0; c->capacity = 0; c->cursor = 0; c->last_sampled = -1;
-    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->launches = 0; c->profiling = false;
+    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->opt_scan = 0; c->launches = 0; c->profiling = false;
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
     c->cline_ok = false; c->cl_CS = 0; c->cl_strips = 0; c->cl_resident = 0;
@@ -459,6 +460,11 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_sweep = value;
         return CH_OK;
     }
+    if (!strcmp(key, "scan")) {
+        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: scan must be 0 (auto), 1 (off) or 2 (always)");
+        ctx->opt_scan = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "rhs3")) {
         if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: rhs3 must be 0 (auto) or 1 (tile kernel)");
         ctx->opt_rhs3 = value;
@@ -545,6 +551,16 @@ static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
     memcpy(p.alpha, c->fac.alpha, sizeof(p.alpha));
     memcpy(p.beta, c->fac.beta, sizeof(p.beta));
     p.W = c->dW; p.K = c->fac.K; p.P = c->fac.P;
+    // log-depth closure (contiguous-line kernels only): worth it once the K-term sum is long
+    p.scan = 0;
+    const int P = c->fac.P;
+    if (c->opt_scan != 1 && (c->fac.K > 4 || c->opt_scan == 2) && P >= 2 && P <= 32 && (P & (P - 1)) == 0) {
+        int lg = 0;
+        while ((1 << lg) < P) ++lg;
+        p.scan = lg;
+        memcpy(p.Mp, c->fac.Mpow2, sizeof(p.Mp));
+        memcpy(p.Wc, c->fac.Wclose, sizeof(p.Wc));
+    }
 }
 
 // axis 0 = x, 1 = y, 2 = z.  update: C += result (last sweep of a step).  scale: multiply the output by oscale.

@@ -92,6 +92,17 @@ int ch_factor_build(ChFactor *f, int N, double sigma, int LC)
         }
     }
     f->K = K;
+    {
+        M2 pw = M;
+        for (int k = 0; k < 7; ++k) {
+            f->Mpow2[k][0] = (double)pw.a; f->Mpow2[k][1] = (double)pw.b; f->Mpow2[k][2] = (double)pw.c; f->Mpow2[k][3] = (double)pw.d;
+            pw = mul(pw, pw);
+        }
+        M2 MP = { 1, 0, 0, 1 };
+        for (int j = 0; j < f->P; ++j) MP = mul(MP, M);
+        const M2 wc = inv_i_minus(MP);
+        f->Wclose[0] = (double)wc.a; f->Wclose[1] = (double)wc.b; f->Wclose[2] = (double)wc.c; f->Wclose[3] = (double)wc.d;
+    }
     M2 close = { 1, 0, 0, 1 };
     if (K == f->P) {
         M2 MP = { 1, 0, 0, 1 };

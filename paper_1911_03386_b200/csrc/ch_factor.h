@@ -30,6 +30,10 @@ struct ChFactor {
     double alpha[CH_MAX_LC];   // homogeneous solutions: u_k for (u_-1,u_-2) = (1,0)
     double beta[CH_MAX_LC];    //                                   ... = (0,1)
     double W[CH_MAX_P][4];     // W_j = M^{j-1} (I - M^P)^-1 (K == P) or M^{j-1} (K < P), row-major 2x2
+    // log-depth closure (warp-shuffle scan over the chunks of a line, used when K is large):
+    // T_{k+1}(c) = T_k(c) + M^(2^k) T_k(c - 2^k) (cyclic), s_in(c) = (I - M^P)^-1 T_log2P(c - 1)
+    double Mpow2[7][4];        // M^(2^k), k = 0..6, row-major 2x2
+    double Wclose[4];          // (I - M^P)^-1
     // generic path (one thread per line): closure of the whole line, (I - T^N)^-1
     double Wline[4];
 };

@@ -20,6 +20,10 @@ struct SweepParams {
     double beta[CH_MAX_LC];
     const double *W;            // device [K][4]
     int K, P;
+    // log-depth closure for contiguous lines (chunks of a line in consecutive lanes): used when scan != 0
+    double Mp[5][4];            // M^(2^k)
+    double Wc[4];               // (I - M^P)^-1
+    int scan;                   // 0, or log2 P (P a power of two, 2 <= P <= 32)
 };
 
 // ------------------------------------------------------------------------------------
@@ -234,6 +238,48 @@ __device__ __forceinline__ void chunk_state_in(const SweepParams &prm, const dou
     }
 }
 
+// Log-depth closure: the P chunks of a line sit in P consecutive lanes (P a power of two <= 32).
+// T_0(c) = out(c); T_{k+1}(c) = T_k(c) + M^(2^k) T_k(c -+ 2^k) with cyclic lane indices, so that
+// T(c) = sum_{j<P} M^j out(c -+ j); state entering chunk c = (I - M^P)^-1 T(c -+ 1).  No shared memory.
+__device__ __forceinline__ void chunk_state_scan(const SweepParams &prm, double oa, double ob, int c, int dir,
+                                                 double &a, double &b)
+{
+    const int P = prm.P;
+    const unsigned full = __activemask();     // every thread of the CTA gets here together; the last warp may be partial
+    double ta = oa, tb = ob;
+    for (int k = 0; k < prm.scan; ++k) {
+        const int src = (c - dir * (1 << k)) & (P - 1);
+        const double ua = __shfl_sync(full, ta, src, P), ub = __shfl_sync(full, tb, src, P);
+        ta = fma(prm.Mp[k][0], ua, fma(prm.Mp[k][1], ub, ta));
+        tb = fma(prm.Mp[k][2], ua, fma(prm.Mp[k][3], ub, tb));
+    }
+    const int src = (c - dir) & (P - 1);
+    const double ua = __shfl_sync(full, ta, src, P), ub = __shfl_sync(full, tb, src, P);
+    a = fma(prm.Wc[0], ua, prm.Wc[1] * ub);
+    b = fma(prm.Wc[2], ua, prm.Wc[3] * ub);
+}
+
+// Same solve as chunk_solve for kernels whose thread index is line * P + chunk (contiguous lines):
+// closure by warp-shuffle scan, no shared memory and no barrier.
+template <int LC>
+__device__ __forceinline__ void chunk_solve_scan(const SweepParams &prm, double (&v)[LC], int c)
+{
+    const double np = prm.np, nq = prm.nq;
+    double a, b;
+    v[1] = fma(np, v[0], v[1]);
+#pragma unroll
+    for (int k = 2; k < LC; ++k) v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k]));
+    chunk_state_scan(prm, v[LC - 1], v[LC - 2], c, +1, a, b);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
+    v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
+#pragma unroll
+    for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
+    chunk_state_scan(prm, v[0], v[1], c, -1, a, b);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
+}
+
 template <int LC>
 __device__ __forceinline__ void chunk_solve(const SweepParams &prm, double (&v)[LC], double *sa, double *sb,
                                             int c, int cstride)
@@ -337,7 +383,8 @@ __global__ void k_sweep_contig(const __grid_constant__ SweepParams prm, double *
         double2 x = live ? sl[swz<LC>(gbase + k)] : make_double2(0.0, 0.0);
         v[2 * k] = x.x; v[2 * k + 1] = x.y;
     }
-    chunk_solve<LC>(prm, v, sa + l * P, sb + l * P, c, 1);
+    if (prm.scan) chunk_solve_scan<LC>(prm, v, c);
+    else chunk_solve<LC>(prm, v, sa + l * P, sb + l * P, c, 1);
     if (live) {
 #pragma unroll
         for (int k = 0; k < LC / 2; ++k) {

@@ -76,6 +76,11 @@ def test_sweep_kernels(B, oracle, N, D, M, sigma):
         got, ref = e.sweep(w, axis), oracle.sweep(w, sigma, axis)
         assert np.abs(got - ref).max() <= tol * np.abs(ref).max(), f"axis {axis}"
     if B.ch_get_option(e.ctx, "chunked"):
+        for scan in (1, 2):                            # K-term sum / warp-shuffle scan closure of the x-sweep
+            B.ch_set_option(e.ctx, "scan", scan)
+            got, ref = e.sweep(w, 0), oracle.sweep(w, sigma, 0)
+            assert np.abs(got - ref).max() <= tol * np.abs(ref).max(), f"scan {scan}"
+        B.ch_set_option(e.ctx, "scan", 0)
         B.ch_set_option(e.ctx, "sweep", 1)             # generic kernels on the same data
         for axis in range(D):
             got, ref = e.sweep(w, axis), oracle.sweep(w, sigma, axis)
