@@ -671,6 +671,15 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
     memcpy(p.W0, c->fac.W[0], sizeof(p.W0));
     memcpy(p.W1, c->fac.W[1], sizeof(p.W1));
     p.W = c->dW; p.K = c->fac.K;
+    p.scan = 0;
+    {
+        const int P = c->fac.P;
+        if (c->opt_scan != 1 && (p.K > 8 || c->opt_scan == 2) && (P & (P - 1)) == 0) {   // measured: the K-term sum wins up to K = 7
+            while ((1 << p.scan) < P) ++p.scan;
+            memcpy(p.Mp, c->fac.Mpow2, sizeof(p.Mp));
+            memcpy(p.Wc, c->fac.Wclose, sizeof(p.Wc));
+        }
+    }
     p.ntiles = c->l_strips * c->M; p.write = write ? 1 : 0;
     const int grid = p.ntiles < c->l_resident ? p.ntiles : c->l_resident;
     const size_t smem = line_smem(c->N);
@@ -695,7 +704,7 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
     memcpy(p.beta, f.beta, sizeof(p.beta));
     memcpy(p.W0, f.W[0], sizeof(p.W0));
     memcpy(p.W1, f.W[1], sizeof(p.W1));
-    p.W = nullptr; p.K = f.K;
+    p.W = nullptr; p.K = f.K; p.scan = 0;
     p.ntiles = c->cl_strips * c->M; p.write = 1;
     const int ncl = p.ntiles < c->cl_resident ? p.ntiles : c->cl_resident;
     cudaLaunchConfig_t cfg = {};

@@ -31,6 +31,9 @@ struct LineParams {
     double W0[4], W1[4];            // first two closure matrices (all of them when K <= 2)
     const double *W;                // device [K][4] (ch_factor.h)
     int K, ntiles, write;
+    // log-depth closure of the barrier kernels when the K-term sum is long (ch_factor.h, Mpow2 / Wclose)
+    double Mp[5][4], Wc[4];
+    int scan;                       // 0, or log2 P (P a power of two)
 };
 
 __device__ __forceinline__ void line_cp_async16(void *smem_dst, const void *gsrc)
@@ -94,6 +97,37 @@ __device__ __forceinline__ void line_state_in(const LineParams &prm, const doubl
         const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
         acc(s, W01.x, W01.y, W23.x, W23.y);
     }
+}
+
+// Log-depth closure for the barrier kernels (after the CTA barrier that follows the slot writes): the
+// slots are re-read TRANSPOSED -- lane = chunk, 32 / P columns per warp pass, two passes cover the 32
+// columns -- scanned with width-P shuffles exactly as chunk_state_scan (ch_kernels.cuh), written back in
+// place as the states ENTERING each chunk, and after one more barrier every thread picks up its own.
+template <int P>
+__device__ __forceinline__ void line_scan_closure(const LineParams &prm, double2 *slots, int tid, int dir,
+                                                  double &aA, double &bA, double &aB, double &bB)
+{
+    constexpr int CPW = 32 / P;
+    const int lane = tid & 31, wid = tid >> 5, ch = lane % P;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const int col = q * 16 + wid * CPW + lane / P;
+        double2 *slot = slots + ((col >> 4) * P + ch) * 16 + (col & 15);
+        const double2 o = *slot;
+        double ta = o.x, tb = o.y;
+        for (int k = 0; k < prm.scan; ++k) {
+            const int src = (ch - dir * (1 << k)) & (P - 1);
+            const double ua = __shfl_sync(0xffffffffu, ta, src, P), ub = __shfl_sync(0xffffffffu, tb, src, P);
+            ta = fma(prm.Mp[k][0], ua, fma(prm.Mp[k][1], ub, ta));
+            tb = fma(prm.Mp[k][2], ua, fma(prm.Mp[k][3], ub, tb));
+        }
+        const int src = (ch - dir) & (P - 1);
+        const double ua = __shfl_sync(0xffffffffu, ta, src, P), ub = __shfl_sync(0xffffffffu, tb, src, P);
+        *slot = make_double2(fma(prm.Wc[0], ua, prm.Wc[1] * ub), fma(prm.Wc[2], ua, prm.Wc[3] * ub));
+    }
+    __syncthreads();
+    const double2 sA = slots[tid], sB = slots[16 * P + tid];
+    aA = sA.x; bA = sA.y; aB = sB.x; bB = sB.y;
 }
 
 // NC = N at compile time (row offsets become immediates).
@@ -237,7 +271,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
         {
             double aA, bA, aB, bB;
-            line_state_in<P>(prm, slotF, tid, +1, aA, bA, aB, bB);
+            if (!NB && (P & (P - 1)) == 0 && prm.scan) line_scan_closure<P>(prm, slotF, tid, +1, aA, bA, aB, bB);
+            else line_state_in<P>(prm, slotF, tid, +1, aA, bA, aB, bB);
 #pragma unroll
             for (int k = 0; k < LC; ++k) {
                 vA[k] = fma(prm.alpha[k], aA, fma(prm.beta[k], bA, vA[k]));
@@ -264,7 +299,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
         {
             double aA, bA, aB, bB;
-            line_state_in<P>(prm, slotB, tid, -1, aA, bA, aB, bB);
+            if (!NB && (P & (P - 1)) == 0 && prm.scan) line_scan_closure<P>(prm, slotB, tid, -1, aA, bA, aB, bB);
+            else line_state_in<P>(prm, slotB, tid, -1, aA, bA, aB, bB);
             // where this thread's results go, recomputed from the tile and thread index
             const int t2 = opaque(tile), tid2 = opaque(tid);
             const int strip2 = t2 % strips, m2 = t2 / strips, li2 = tid2 & 15;
