@@ -26,6 +26,17 @@ struct SweepParams {
     int scan;                   // 0, or log2 P (P a power of two, 2 <= P <= 32)
 };
 
+// 16-byte asynchronous global -> shared copy (L2 only), and its group fences
+__device__ __forceinline__ void ck_cp_async16(void *smem_dst, const void *gsrc)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void ck_cp_async_wait_all()
+{
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
+}
+
 // ------------------------------------------------------------------------------------
 // reductions
 // ------------------------------------------------------------------------------------
@@ -371,7 +382,8 @@ __global__ void k_sweep_contig(const __grid_constant__ SweepParams prm, double *
     double *sa = reinterpret_cast<double *>(sl + (size_t)LPB * (N / 2));
     double *sb = sa + LPB * P;
 
-    for (int g = t; g < G; g += nthreads) sl[swz<LC>(g)] = g2[g];
+    for (int g = t; g < G; g += nthreads) ck_cp_async16(&sl[swz<LC>(g)], g2 + g);
+    ck_cp_async_wait_all();
     __syncthreads();
 
     const int l = t / P, c = t - l * P;
