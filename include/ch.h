@@ -145,6 +145,26 @@ const char *ch_kernel_kind_name(int kind);
 /* Kernel launches enqueued by this context since creation (each graph node counts once per replay). */
 long long ch_launch_count(const ch_ctx *ctx);
 
+/* ---- Ensemble statistics of the coarsening rate (off the hot path) ----
+ * Input everywhere: the series buffer ch_step writes, series[nsamples][ensemble][4] = {F, dF/dt, beta, mass},
+ * on the device.  Members gathered from several ranks are simply concatenated along the member axis first.
+ * All calls are asynchronous on `stream` (a cudaStream_t, NULL = default stream); outputs are device pointers
+ * owned by the caller.  Return CH_OK, CH_EINVAL (null pointer, sizes < 1, bad window or bins), CH_ECUDA.
+ *
+ * ch_stats_moments: eq. (41a,b): moments[s] = {mu_1, mu_2, mu_3, mu_4} of beta over the members at
+ *   sample s, mu_1 = (1/M) sum_j beta_j, mu_p = (1/M) sum_j (beta_j - mu_1)^p.  moments_dev is [nsamples][4].
+ * ch_stats_hist: histogram of beta at every sample time (Figs 9, 14, 18): hist[s][b] = number of members with
+ *   floor((beta - lo) / width) == b, 0 <= b < nbins (values outside are dropped).  hist_dev is int[nsamples][nbins].
+ * ch_stats_fit: over the samples with t1 <= t_s <= t2, t_s = t0 + s * dt_sample: out[0] = beta_0, the time average of
+ *   mu_1 (eq. (42); trapezoid rule over the samples, divided by the span they cover), out[1] = k, the
+ *   least-squares slope of mu_2 = k t through the origin, k = sum t mu_2 / sum t^2, out[2] = number of
+ *   samples in the window.  moments_dev is the output of ch_stats_moments; out_dev is double[3]. */
+int ch_stats_moments(const double *series_dev, int nsamples, int ensemble, double *moments_dev, void *stream);
+int ch_stats_hist(const double *series_dev, int nsamples, int ensemble, double lo, double width, int nbins,
+                  int *hist_dev, void *stream);
+int ch_stats_fit(const double *moments_dev, int nsamples, double t0, double dt_sample, double t1, double t2,
+                 double *out_dev, void *stream);
+
 /* Message for the last error on this context (never NULL); ch_create failures: pass NULL. */
 const char *ch_last_error(const ch_ctx *ctx);
 

@@ -20,7 +20,7 @@ EXPORTS = [
     "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_energy", "ch_get_state",
     "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
     "ch_launch_count", "ch_last_error", "ch_profile", "ch_profile_read", "ch_kernel_kinds",
-    "ch_kernel_kind_name",
+    "ch_kernel_kind_name", "ch_stats_moments", "ch_stats_hist", "ch_stats_fit",
 ]
 
 _LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libch.so")
@@ -68,6 +68,9 @@ def lib():
         L.ch_kernel_kinds.restype = ci
         L.ch_kernel_kind_name.argtypes = [ci]
         L.ch_kernel_kind_name.restype = ctypes.c_char_p
+        L.ch_stats_moments.argtypes = [dp, ci, ci, dp, vp]
+        L.ch_stats_hist.argtypes = [dp, ci, ci, cd, cd, ci, vp, vp]
+        L.ch_stats_fit.argtypes = [dp, ci, cd, cd, cd, cd, dp, vp]
         L.ch_last_error.argtypes = [vp]
         L.ch_last_error.restype = ctypes.c_char_p
         _lib = L
@@ -186,6 +189,32 @@ def ch_profile_read(ctx):
     cnt = (ctypes.c_longlong * n)()
     _check(ctx, lib().ch_profile_read(ctx, ms, cnt, n))
     return {lib().ch_kernel_kind_name(k).decode(): (ms[k], cnt[k]) for k in range(n)}
+
+
+def _stats_check(rc, what):
+    if rc != CH_OK:
+        raise ChError(rc, what)
+
+
+def ch_stats_moments(series, moments, stream=None):
+    """series: CUDA tensor [S][M][4]; moments: CUDA tensor [S][4] (output)."""
+    S, M = series.shape[0], series.shape[1]
+    assert series.is_cuda and moments.is_cuda and series.is_contiguous() and tuple(moments.shape) == (S, 4)
+    _stats_check(lib().ch_stats_moments(series.data_ptr(), S, M, moments.data_ptr(), ctypes.c_void_p(stream or 0)), "ch_stats_moments")
+
+
+def ch_stats_hist(series, lo, width, nbins, hist, stream=None):
+    """hist: CUDA int32 tensor [S][nbins] (output)."""
+    S, M = series.shape[0], series.shape[1]
+    assert series.is_cuda and hist.is_cuda and series.is_contiguous() and tuple(hist.shape) == (S, nbins)
+    _stats_check(lib().ch_stats_hist(series.data_ptr(), S, M, lo, width, nbins, hist.data_ptr(), ctypes.c_void_p(stream or 0)), "ch_stats_hist")
+
+
+def ch_stats_fit(moments, t0, dt_sample, t1, t2, out, stream=None):
+    """out: CUDA tensor [3] = {beta_0, k, samples in the window} (output)."""
+    assert moments.is_cuda and out.is_cuda and out.numel() == 3
+    _stats_check(lib().ch_stats_fit(moments.data_ptr(), moments.shape[0], t0, dt_sample, t1, t2, out.data_ptr(),
+                                    ctypes.c_void_p(stream or 0)), "ch_stats_fit")
 
 
 # ---- convenience wrapper ---------------------------------------------------------------

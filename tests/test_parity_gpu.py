@@ -392,3 +392,62 @@ def test_attached_workspace_and_device_pointers(B):
     assert np.array_equal(en.cpu().numpy(), sref[-1])
     assert B.ch_launch_count(e.ctx) > 0
     e.close()
+
+
+# ---------------------------------------------------- ensemble statistics
+def test_ensemble_statistics_against_the_oracle(B, oracle):
+    """eq. (41), (42), P:548 on a real series: 48 members x 128^2 (mixed mixtures), 600 steps sampled every 20;
+    moments, window average, slope and histogram against oracle/stats_oracle.py; integer counts bit-exact."""
+    import torch
+    from oracle import stats_oracle as so
+    M, N = 48, 128
+    C0 = inputs.initial_state(range(7000, 7000 + M), N, 2, [0.0, -0.4] * (M // 2), 0.05)
+    e = B.Ensemble(M, N, 2, 1.0, 0.01)
+    e.set_state(C0)
+    e.set_series(20, 31)
+    e.step(600)
+    series = e._series[: B.ch_series_count(e.ctx)].contiguous()
+    S = series.shape[0]
+    assert S == 31
+    mom = torch.empty((S, 4), dtype=torch.float64, device="cuda")
+    hist = torch.empty((S, 40), dtype=torch.int32, device="cuda")
+    fit = torch.empty(3, dtype=torch.float64, device="cuda")
+    B.ch_stats_moments(series, mom)
+    B.ch_stats_hist(series, -0.05, 0.0125, 40, hist)
+    B.ch_stats_fit(mom, 0.0, 0.2, 2.0, 5.0, fit)
+    torch.cuda.synchronize()
+    sh = series.cpu().numpy()
+    e.close()
+    ref = so.moments(sh)
+    got = mom.cpu().numpy()
+    scale = np.abs(sh[:, :, 2]).max(axis=1)[:, None] ** np.arange(1, 5)[None, :] + 1e-300
+    assert (np.abs(got - ref) / scale).max() <= 1e-12
+    assert np.array_equal(hist.cpu().numpy(), so.hist(sh, -0.05, 0.0125, 40))
+    f = fit.cpu().numpy()
+    assert abs(f[0] - so.beta0(ref, 0.0, 0.2, 2.0, 5.0)) <= 1e-12 * max(1e-3, abs(f[0]))
+    assert abs(f[1] - so.slope_k(ref, 0.0, 0.2, 2.0, 5.0)) <= 1e-12 * max(1e-6, abs(f[1]))
+    assert f[2] == 16
+
+
+def test_ensemble_statistics_edge_cases(B):
+    import torch
+    from oracle import stats_oracle as so
+    rng = np.random.default_rng(2)
+    for S, M in [(1, 1), (3, 2), (5, 1000), (2, 257)]:
+        sh = rng.normal(0.3, 0.1, size=(S, M, 4))
+        series = torch.from_numpy(sh).cuda()
+        mom = torch.empty((S, 4), dtype=torch.float64, device="cuda")
+        hist = torch.empty((S, 7), dtype=torch.int32, device="cuda")
+        fit = torch.empty(3, dtype=torch.float64, device="cuda")
+        B.ch_stats_moments(series, mom)
+        B.ch_stats_hist(series, 0.0, 0.1, 7, hist)
+        B.ch_stats_fit(mom, 1.0, 0.5, 0.0, 100.0, fit)
+        torch.cuda.synchronize()
+        ref = so.moments(sh)
+        assert np.allclose(mom.cpu().numpy(), ref, rtol=1e-11, atol=1e-17)
+        assert np.array_equal(hist.cpu().numpy(), so.hist(sh, 0.0, 0.1, 7))
+        f = fit.cpu().numpy()
+        assert np.isclose(f[0], so.beta0(ref, 1.0, 0.5, 0.0, 100.0), rtol=1e-12)
+        assert np.isclose(f[1], so.slope_k(ref, 1.0, 0.5, 0.0, 100.0), rtol=1e-12)
+    with pytest.raises(B.ChError):
+        B.ch_stats_hist(series, 0.0, -1.0, 7, hist)
