@@ -306,6 +306,25 @@ def test_determinism_and_member_independence(B):
     assert np.array_equal(one[0], a[3]) and np.array_equal(s1[:, 0], sa[:, 3])   # ensemble size
 
 
+@pytest.mark.parametrize("M,N,steps", [(40, 512, 30), (6, 1024, 20), (3, 2048, 10)])
+def test_flag_synchronised_kernels_are_deterministic_and_match_three_pass(B, M, N, steps):
+    """The line kernel (N = 512: more tiles than resident CTAs) and the cluster line kernel (N = 1024, 2048)
+    synchronise warps and CTAs with release/acquire flags instead of barriers: repeated runs must agree
+    bitwise, and agree with the barrier-synchronised variants and the three-pass step to round-off."""
+    C0 = inputs.initial_state(range(500, 500 + M), N, 2, -0.3, 0.1)
+    a, sa = run_gpu(B, C0, 1.0, 0.01, steps, 10)
+    for _ in range(3):
+        b, sb = run_gpu(B, C0, 1.0, 0.01, steps, 10)
+        assert np.array_equal(a, b) and np.array_equal(sa, sb)
+    ref, sr = run_gpu(B, C0, 1.0, 0.01, steps, 10, options={"fuse": 1})
+    assert np.abs(a - ref).max() <= 1e-13
+    assert_series_close(sa, sr, 1e-12)
+    alt = {"fuse": 3, "linesync": 1} if N == 512 else {"fuse": 2}
+    c, sc = run_gpu(B, C0, 1.0, 0.01, steps, 10, options=alt)
+    assert np.abs(a - c).max() <= 1e-13
+    assert_series_close(sa, sc, 1e-12)
+
+
 def test_equivariances_on_gpu(B):
     C0 = inputs.initial_state([3, 4], 128, 2, [0.0, -0.3], 0.2)
     base, _ = run_gpu(B, C0, 1.0, 0.01, 50, 50)
