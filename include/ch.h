@@ -165,6 +165,14 @@ int ch_stats_hist(const double *series_dev, int nsamples, int ensemble, double l
 int ch_stats_fit(const double *moments_dev, int nsamples, double t0, double dt_sample, double t1, double t2,
                  double *out_dev, void *stream);
 
+/* ch_grid_doubling_error: the self-convergence measure of eq. (A.1), P:672-674:
+ *   out[m] = (1/|Omega|) sum_{i,j} | (1/4) (the four fine-grid values in coarse cell (i,j)) - coarse[m][i][j] | dx_c^2
+ *          = (1/n_coarse^2) sum_{i,j} | ... |
+ * for 2D fields fine[ensemble][2 n_coarse][2 n_coarse] and coarse[ensemble][n_coarse][n_coarse] on cell-centred grids
+ * of the same periodic domain (device pointers, caller-owned; out_dev is double[ensemble]); asynchronous on stream. */
+int ch_grid_doubling_error(const double *fine_dev, const double *coarse_dev, int ensemble, int n_coarse,
+                           double *out_dev, void *stream);
+
 /* Message for the last error on this context (never NULL); ch_create failures: pass NULL. */
 const char *ch_last_error(const ch_ctx *ctx);
 

@@ -6,6 +6,7 @@ __graft_entry__.smoke() and bench.py's cpu_baseline leg may import it.
     beta0     eq. (42), P:460          (1 / (t2 - t1)) int_{t1}^{t2} mu_1 dt
     slope_k   P:548                    least-squares fit of mu_2(t) to the trend line mu_2 = k t
     hist      Figs 9, 14, 18           histogram of beta over the members at each sample time
+    grid_doubling_error  eq. (A.1), P:672-674   (1/|Omega|) sum |mean of the 4 fine values in a coarse cell - coarse value| dx_c^2
 
 Readings (G18-G20): the integral of eq. (42) is the trapezoid rule over the stored
 samples inside the window, divided by the time span those samples cover; the trend line goes through the
@@ -61,3 +62,18 @@ def hist(series, lo, width, nbins):
             if 0 <= q < nbins:
                 out[s, int(q)] += 1
     return out
+
+
+def grid_doubling_error(fine, coarse):
+    """eq. (A.1): fine[M][2n][2n], coarse[M][n][n] -> E[M]; |Omega| = n^2 dx_c^2, so E = sum|.| / n^2."""
+    fine, coarse = np.asarray(fine, dtype=np.float64), np.asarray(coarse, dtype=np.float64)
+    M, n = coarse.shape[0], coarse.shape[1]
+    E = np.zeros(M)
+    for m in range(M):
+        total = 0.0
+        for i in range(n):
+            for j in range(n):
+                avg = 0.25 * (fine[m, 2 * i, 2 * j] + fine[m, 2 * i, 2 * j + 1] + fine[m, 2 * i + 1, 2 * j] + fine[m, 2 * i + 1, 2 * j + 1])
+                total += abs(avg - coarse[m, i, j])
+        E[m] = total / (n * n)
+    return E

@@ -20,7 +20,7 @@ EXPORTS = [
     "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_energy", "ch_get_state",
     "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
     "ch_launch_count", "ch_last_error", "ch_profile", "ch_profile_read", "ch_kernel_kinds",
-    "ch_kernel_kind_name", "ch_stats_moments", "ch_stats_hist", "ch_stats_fit",
+    "ch_kernel_kind_name", "ch_stats_moments", "ch_stats_hist", "ch_stats_fit", "ch_grid_doubling_error",
 ]
 
 _LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libch.so")
@@ -71,6 +71,7 @@ def lib():
         L.ch_stats_moments.argtypes = [dp, ci, ci, dp, vp]
         L.ch_stats_hist.argtypes = [dp, ci, ci, cd, cd, ci, vp, vp]
         L.ch_stats_fit.argtypes = [dp, ci, cd, cd, cd, cd, dp, vp]
+        L.ch_grid_doubling_error.argtypes = [dp, dp, ci, ci, dp, vp]
         L.ch_last_error.argtypes = [vp]
         L.ch_last_error.restype = ctypes.c_char_p
         _lib = L
@@ -215,6 +216,15 @@ def ch_stats_fit(moments, t0, dt_sample, t1, t2, out, stream=None):
     assert moments.is_cuda and out.is_cuda and out.numel() == 3
     _stats_check(lib().ch_stats_fit(moments.data_ptr(), moments.shape[0], t0, dt_sample, t1, t2, out.data_ptr(),
                                     ctypes.c_void_p(stream or 0)), "ch_stats_fit")
+
+
+def ch_grid_doubling_error(fine, coarse, out, stream=None):
+    """fine: CUDA tensor [M][2n][2n], coarse: [M][n][n], out: [M] (output): eq. (A.1)."""
+    M, n = coarse.shape[0], coarse.shape[1]
+    assert fine.is_cuda and coarse.is_cuda and out.is_cuda and fine.is_contiguous() and coarse.is_contiguous()
+    assert tuple(fine.shape) == (M, 2 * n, 2 * n) and tuple(coarse.shape) == (M, n, n) and out.numel() == M
+    _stats_check(lib().ch_grid_doubling_error(fine.data_ptr(), coarse.data_ptr(), M, n, out.data_ptr(),
+                                              ctypes.c_void_p(stream or 0)), "ch_grid_doubling_error")
 
 
 # ---- convenience wrapper ---------------------------------------------------------------

@@ -105,3 +105,35 @@ extern "C" int ch_stats_fit(const double *moments_dev, int nsamples, double t0, 
     k_stats_fit<<<1, 32, 0, (cudaStream_t)stream>>>(moments_dev, nsamples, t0, dt_sample, t1, t2, out_dev);
     return cudaGetLastError() == cudaSuccess ? CH_OK : CH_ECUDA;
 }
+
+// ---- grid-doubling self-convergence error, eq. (A.1) P:672-674 ----
+// E[m] = (1 / nc^2) sum_{i,j < nc} | (1/4)(f[2i][2j] + f[2i][2j+1] + f[2i+1][2j] + f[2i+1][2j+1]) - c[i][j] |
+// (|Omega| = nc^2 dx_c^2 cancels the cell area).  One CTA per member, fixed summation order.
+__global__ void __launch_bounds__(1024) k_grid_doubling_error(const double *__restrict__ fine, const double *__restrict__ coarse,
+                                                              int nc, double *__restrict__ out)
+{
+    __shared__ double red[1024];
+    const int m = blockIdx.x, t = threadIdx.x, nf = 2 * nc;
+    const double *f = fine + (size_t)m * nf * nf, *c = coarse + (size_t)m * nc * nc;
+    double acc = 0.0;
+    for (long long p = t; p < (long long)nc * nc; p += 1024) {
+        const int i = (int)(p / nc), j = (int)(p - (long long)i * nc);
+        const double *q = f + (size_t)(2 * i) * nf + 2 * j;
+        acc += fabs(0.25 * ((q[0] + q[1]) + (q[nf] + q[nf + 1])) - c[p]);
+    }
+    red[t] = acc;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (t < o) red[t] += red[t + o];
+        __syncthreads();
+    }
+    if (t == 0) out[m] = red[0] / ((double)nc * nc);
+}
+
+extern "C" int ch_grid_doubling_error(const double *fine_dev, const double *coarse_dev, int ensemble, int n_coarse,
+                                      double *out_dev, void *stream)
+{
+    if (!fine_dev || !coarse_dev || !out_dev || ensemble < 1 || n_coarse < 1 || n_coarse > 16384) return CH_EINVAL;
+    k_grid_doubling_error<<<ensemble, 1024, 0, (cudaStream_t)stream>>>(fine_dev, coarse_dev, n_coarse, out_dev);
+    return cudaGetLastError() == cudaSuccess ? CH_OK : CH_ECUDA;
+}

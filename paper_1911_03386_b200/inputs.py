@@ -65,3 +65,15 @@ def config_state(name: str, members=None) -> np.ndarray:
     cb = c["cbar"]
     cbars = [cb[k] for k in idx] if isinstance(cb, (list, tuple)) else [cb] * len(idx)
     return initial_state([c["seed0"] + k for k in idx], c["N"], c["D"], cbars, c["amp"])
+
+
+def droplet_state(n: int, L: float, gamma: float, a: float, b: float) -> np.ndarray:
+    """Single elliptical droplet for the grid-doubling study of the paper's Appendix A.  The
+    printed IC is garbled (reading G13): a circular tanh droplet is stationary (only the O(h^2)
+    spatial error would show) and a 1e-6-amplitude seed grows chaotically, so the study uses a droplet that
+    EVOLVES smoothly: an ellipse with semi-axes (a, b) relaxing towards a circle,
+    C0 = tanh((1 - rho) sqrt(a b) / sqrt(2 gamma)), rho^2 = ((x - L/2)/a)^2 + ((y - L/2)/b)^2,
+    sampled on the cell-centred n x n grid x_i = (i + 1/2) L / n of [0, L]^2.  Shape [1][n][n]."""
+    x = (np.arange(n) + 0.5) * (L / n)
+    rho = np.sqrt(((x[None, :] - 0.5 * L) / a) ** 2 + ((x[:, None] - 0.5 * L) / b) ** 2)
+    return np.tanh((1.0 - rho) * np.sqrt(a * b) / np.sqrt(2.0 * gamma))[None]

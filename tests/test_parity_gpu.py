@@ -470,3 +470,41 @@ def test_ensemble_statistics_edge_cases(B):
         assert np.isclose(f[1], so.slope_k(ref, 1.0, 0.5, 0.0, 100.0), rtol=1e-12)
     with pytest.raises(B.ChError):
         B.ch_stats_hist(series, 0.0, -1.0, 7, hist)
+
+
+# ---------------------------------------------------- grid-doubling convergence
+def test_grid_doubling_error_kernel(B):
+    import torch
+    from oracle import stats_oracle as so
+    rng = np.random.default_rng(4)
+    for M, n in [(1, 1), (3, 8), (2, 37), (1, 256)]:
+        fine, coarse = rng.standard_normal((M, 2 * n, 2 * n)), rng.standard_normal((M, n, n))
+        out = torch.empty(M, dtype=torch.float64, device="cuda")
+        B.ch_grid_doubling_error(torch.from_numpy(fine).cuda(), torch.from_numpy(coarse).cuda(), out)
+        assert np.allclose(out.cpu().numpy(), so.grid_doubling_error(fine, coarse), rtol=1e-12)
+
+
+def test_grid_doubling_study_first_order_and_oracle_parity(B, oracle):
+    """Appendix A: elliptical droplet on [0, 2 pi]^2, gamma = 0.01, dt = 0.1 dx, T = 10
+    (gamma dt / dx^4 = 2.1 at n = 128 ... 1082 at n = 1024).  The n = 128 run is checked against the oracle
+    step by step in the rescaled h = 1 units.  Error = O(dx^2) + O(dt) with dt ~ dx: the observed order
+    log2(E_n / E_2n) must fall from 2 towards 1; halving dt at fixed n isolates the first order in time."""
+    import math
+    import torch
+    from paper_1911_03386_b200 import convergence as cv
+    from oracle import stats_oracle as so
+    L = 2 * math.pi
+    g, d, nsteps = cv.scaled_parameters(128, L, 0.01, 10.0, 0.1)
+    Co, _ = oracle.run(inputs.droplet_state(128, L, 0.01, 1.8, 0.9), g, d, nsteps, nsteps)
+    f128 = cv.final_state(128).cpu().numpy()
+    assert np.abs(f128 - Co).max() <= FIELD_TOL
+    rows = cv.study([128, 256, 512, 1024])
+    ns, E, order = zip(*rows)
+    assert ns == (256, 512, 1024)
+    assert E[0] > E[1] > E[2] > 0                                   # converges
+    assert 1.0 <= order[2] < order[1] <= 2.05, rows                  # between first and second order, falling
+    assert abs(E[0] - so.grid_doubling_error(cv.final_state(256).cpu().numpy(), f128)[0]) <= 1e-12
+    # time refinement at fixed n = 256: differences of successive halvings of dt halve (first order, P:684)
+    a, b, c = (cv.final_state(256, dt_factor=f) for f in (0.2, 0.1, 0.05))
+    d1, d2 = float((a - b).abs().mean()), float((b - c).abs().mean())
+    assert 0.9 <= math.log2(d1 / d2) <= 1.1, (d1, d2)

@@ -82,3 +82,25 @@ def test_hist_against_numpy_histogram_and_edges():
     # left edge belongs to the bin, right end is open, outside values are dropped
     b = np.array([[0.0, 0.25, 0.5, 0.999999, 1.0, -1e-9]])
     assert so.hist(series_from_beta(b), 0.0, 0.25, 4)[0].tolist() == [1, 1, 1, 1]
+
+
+def test_grid_doubling_error_closed_forms():
+    """eq. (A.1), P:672-674 on cell-centred grids: a linear field has E = 0 (the mean of the four fine
+    samples IS the coarse sample); f = x^2 + y^2 has E = h_f^2 / 2 exactly; a constant offset d gives |d|."""
+    n, L = 8, 2.0
+    hf, hc = L / (2 * n), L / n
+    xf, xc = (np.arange(2 * n) + 0.5) * hf, (np.arange(n) + 0.5) * hc
+    lin_f = (3.0 * xf[None, :] - 2.0 * xf[:, None] + 0.7)[None]
+    lin_c = (3.0 * xc[None, :] - 2.0 * xc[:, None] + 0.7)[None]
+    assert so.grid_doubling_error(lin_f, lin_c)[0] <= 1e-15
+    q_f = (xf[None, :] ** 2 + xf[:, None] ** 2)[None]
+    q_c = (xc[None, :] ** 2 + xc[:, None] ** 2)[None]
+    assert abs(so.grid_doubling_error(q_f, q_c)[0] - hf ** 2 / 2) <= 1e-14
+    assert abs(so.grid_doubling_error(lin_f, lin_c - 0.25)[0] - 0.25) <= 1e-15
+    # transposed operands / wrong 2x2 block fail: an x-only field against its y-only twin
+    fx = np.tile(xf[None, :], (2 * n, 1))[None]
+    assert so.grid_doubling_error(fx, np.tile(xc[None, :], (n, 1))[None])[0] <= 1e-15
+    assert so.grid_doubling_error(fx, np.tile(xc[:, None], (1, n))[None])[0] > 0.1
+    # members are independent
+    two = so.grid_doubling_error(np.concatenate([lin_f, q_f]), np.concatenate([lin_c, q_c]))
+    assert two[0] <= 1e-15 and abs(two[1] - hf ** 2 / 2) <= 1e-14
