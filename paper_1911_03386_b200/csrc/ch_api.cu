@@ -33,6 +33,7 @@ struct ch_ctx {
     bool chunked;           // chunked sweeps available for this N
     int LC;
     double *dW;             // device copy of fac.W
+    double *dW16;           // device copy of fac16.W (cluster line mode when c->LC is 32), else NULL
     double rscale;          // dt / c0^D: the 1/c0 of every sweep folded into the RHS
     // device arrays
     void *ws_base;          // cudaMalloc'ed or attached
@@ -234,7 +235,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         return fail(nullptr, CH_EINVAL, "ch_create: factorisation of I + gamma dt (delta^2)^2 failed its self-check");
     }
     c->rscale = dt / std::pow(c->fac.c0, D);
-    c->dW = nullptr;
+    c->dW = nullptr; c->dW16 = nullptr;
     c->nparts = rhs_parts(N, D);
     if (D == 2) { c->rhs_tiles_x = (N + RHS2_TX - 1) / RHS2_TX; c->rhs_tiles_y = (N + RHS2_TY - 1) / RHS2_TY; }
     else { c->rhs_tiles_x = (N + RHS3_TX - 1) / RHS3_TX; c->rhs_tiles_y = (N + RHS3_TY - 1) / RHS3_TY; }
@@ -265,6 +266,12 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
             if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<4>, &cfg);
         }
         if (e == cudaSuccess && ncl >= 1) { c->cline_ok = true; c->cl_resident = ncl; }
+        if (c->cline_ok && c->LC != LINE_LC) {
+            // the x-sweep of the cluster line step also runs at chunk length 16 (69 registers instead of 123)
+            e = cudaMalloc((void **)&c->dW16, sizeof(double) * 4 * CH_MAX_P);
+            if (e == cudaSuccess) e = cudaMemcpy(c->dW16, c->fac16.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { if (c->dW16) cudaFree(c->dW16); c->dW16 = nullptr; }
+        }
         cudaGetLastError();
     }
     c->r3_parts = 0; c->r3_resident = 0; c->opt_rhs3 = 0;
@@ -353,6 +360,7 @@ extern "C" int ch_destroy(ch_ctx *ctx)
     prof_clear(ctx);
     if (ctx->ws_owned && ctx->ws_base) cudaFree(ctx->ws_base);
     if (ctx->dW) cudaFree(ctx->dW);
+    if (ctx->dW16) cudaFree(ctx->dW16);
     delete ctx;
     return CH_OK;
 }
@@ -749,7 +757,14 @@ static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
     SweepParams prm;
     // the line kernels leave the RHS scale dt / c0^2 to this kernel's final fused multiply-add
     fill_params(c, prm, unscaled ? c->rscale : 1.0);
-    const int N = c->N, P = c->fac.P;
+    int LC = c->LC;
+    if (fuse_mode(c) == 4 && c->dW16) {
+        memcpy(prm.alpha, c->fac16.alpha, sizeof(prm.alpha));
+        memcpy(prm.beta, c->fac16.beta, sizeof(prm.beta));
+        prm.W = c->dW16; prm.K = c->fac16.K; prm.P = c->fac16.P; prm.scan = 0;
+        LC = LINE_LC;
+    }
+    const int N = c->N, P = prm.P;
     const long long total_lines = (long long)c->M * N;
     int threads = 256;
     if (P > threads) threads = P;
@@ -758,7 +773,7 @@ static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
     threads = LPB * P;
     const int blocks = (int)((total_lines + LPB - 1) / LPB);
     const size_t smem = (size_t)2 * LPB * N * 8 + (size_t)2 * LPB * P * 8;
-    if (c->LC == 16) k_sweep_x_update<16><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
+    if (LC == 16) k_sweep_x_update<16><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
     else k_sweep_x_update<32><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
 }
 
