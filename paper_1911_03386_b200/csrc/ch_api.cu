@@ -247,7 +247,8 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
     c->cline_ok = false; c->cl_CS = 0; c->cl_strips = 0; c->cl_resident = 0;
-    if (D == 2 && c->fused_ok && (N == 1024 || N == 2048) && ch_factor_build(&c->fac16, N, gamma * dt, LINE_LC) == 0
+    // (the chunk tables of a truncated closure do not depend on N: build them at a line length ch_factor allows)
+    if (D == 2 && (N == 1024 || N == 2048 || N == 4096) && ch_factor_build(&c->fac16, N < 2048 ? N : 2048, gamma * dt, LINE_LC) == 0
         && c->fac16.K <= 2) {
         c->cl_CS = N / CLINE_NC; c->cl_strips = (N + LINE_VALID - 1) / LINE_VALID;
         cudaLaunchConfig_t cfg = {};
@@ -261,12 +262,15 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         if (c->cl_CS == 2) {
             e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
             if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<2>, &cfg);
-        } else {
+        } else if (c->cl_CS == 4) {
             e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
             if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<4>, &cfg);
+        } else {
+            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<8>, &cfg);
         }
         if (e == cudaSuccess && ncl >= 1) { c->cline_ok = true; c->cl_resident = ncl; }
-        if (c->cline_ok && c->LC != LINE_LC) {
+        if (c->cline_ok && c->LC != LINE_LC && N / LINE_LC <= CH_MAX_P) {
             // the x-sweep of the cluster line step also runs at chunk length 16 (69 registers instead of 123)
             e = cudaMalloc((void **)&c->dW16, sizeof(double) * 4 * CH_MAX_P);
             if (e == cudaSuccess) e = cudaMemcpy(c->dW16, c->fac16.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
@@ -485,7 +489,7 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
     }
     if (!strcmp(key, "fuse")) {
         if (value < 0 || value > 4) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line) or 4 (cluster line)");
-        if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2, N in {1024, 2048} and a closure truncated to 2 chunks");
+        if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2, N in {1024, 2048, 4096} and a closure truncated to 2 chunks");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
         if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 192, 256, 384, 512}");
         ctx->opt_fuse = value;
@@ -722,19 +726,33 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
     cfg.gridDim = dim3(c->cl_CS * ncl); cfg.blockDim = dim3(CLINE_NC); cfg.dynamicSmemBytes = cline_smem();
     cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = 1;
     if (c->cl_CS == 2) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<2>, p, (const double *)c->C, c->w);
-    else cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<4>, p, (const double *)c->C, c->w);
+    else if (c->cl_CS == 4) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<4>, p, (const double *)c->C, c->w);
+    else cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<8>, p, (const double *)c->C, c->w);
 }
 
 // number of F/Fdot/mass partials per member the fused RHS kernel in use writes
-static int fused_parts(const ch_ctx *c) { return fuse_mode(c) == 3 ? c->l_strips : c->f_strips * c->f_CS; }
+static int fused_parts(const ch_ctx *c)
+{
+    const int mode = fuse_mode(c);
+    return mode == 3 ? c->l_strips : (mode == 4 ? c->nparts : c->f_strips * c->f_CS);
+}
 
 // diag: also reduce F, Fdot, mass of C^n into the partials; write == false (diag only): no sweep, w untouched.
 // Returns true when w is left WITHOUT the RHS scale dt / c0^2 (k_sweep_x_update then applies it).
 static bool launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
 {
+    if (fuse_mode(c) == 4) {
+        // cluster line step: the sampling reduction is a diagnostics-only launch of the tile RHS kernel
+        // (reads C once more on the 1-in-stride sampling steps), the step itself never changes kernel
+        if (diag) launch_rhs(c, c->C, c->w, c->rscale, true, false);
+        if (write) {
+            ProfScope ps(c, KIND_RHS_SWEEP_Y);
+            launch_rhs_sweep_y_cline(c);
+        }
+        return true;
+    }
     ProfScope ps(c, diag ? KIND_RHS_SWEEP_Y_DIAG : KIND_RHS_SWEEP_Y);
     if (fuse_mode(c) == 3) { launch_rhs_sweep_y_line(c, diag, write); return true; }
-    if (fuse_mode(c) == 4 && !diag) { launch_rhs_sweep_y_cline(c); return true; }
     SweepParams prm;
     fill_params(c, prm, 1.0);
     if (c->LC == 16) { if (diag) launch_rhs_sweep_y_t<16, true>(c, prm, write); else launch_rhs_sweep_y_t<16, false>(c, prm, 1); }

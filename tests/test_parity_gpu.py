@@ -211,6 +211,19 @@ def test_cfg5_long_lines_one_member(B, oracle):
     assert_series_close(s[:, [5]], so)
 
 
+def test_4096_lines_cluster_of_eight(B, oracle):
+    """The paper's largest grid (n = 4096): cluster line kernel with 8 CTAs per line, sampling through
+    the tile RHS kernel; one member, 6 steps sampled every 3, against the oracle."""
+    C0 = inputs.initial_state([4242], 4096, 2, -0.2, 0.05)
+    e = B.Ensemble(1, 4096, 2, 1.0, 0.01)
+    assert B.ch_get_option(e.ctx, "fuse_mode") == 4
+    e.close()
+    C, s = run_gpu(B, C0, 1.0, 0.01, 6, 3)
+    Co, so = oracle.run(C0, 1.0, 0.01, 6, 3)
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+
+
 def test_restart_parity_from_developed_state(B, oracle):
     """cbar = -0.4 is still linear at step 1000, so also compare from a coarsening state:
     GPU runs 10000 steps, the state is handed to both sides, compared after 1000 more."""
