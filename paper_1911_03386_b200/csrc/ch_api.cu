@@ -33,6 +33,7 @@ struct ch_ctx {
     bool chunked;           // chunked sweeps available for this N
     int LC;
     double *dW;             // device copy of fac.W
+    double *dS2;            // device copy of fac.Mlane, fac.WG (two-level scan closure)
     double *dW16;           // device copy of fac16.W (cluster line mode when c->LC is 32), else NULL
     double rscale;          // dt / c0^D: the 1/c0 of every sweep folded into the RHS
     // device arrays
@@ -235,7 +236,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         return fail(nullptr, CH_EINVAL, "ch_create: factorisation of I + gamma dt (delta^2)^2 failed its self-check");
     }
     c->rscale = dt / std::pow(c->fac.c0, D);
-    c->dW = nullptr; c->dW16 = nullptr;
+    c->dW = nullptr; c->dW16 = nullptr; c->dS2 = nullptr;
     c->nparts = rhs_parts(N, D);
     if (D == 2) { c->rhs_tiles_x = (N + RHS2_TX - 1) / RHS2_TX; c->rhs_tiles_y = (N + RHS2_TY - 1) / RHS2_TY; }
     else { c->rhs_tiles_x = (N + RHS3_TX - 1) / RHS3_TX; c->rhs_tiles_y = (N + RHS3_TY - 1) / RHS3_TY; }
@@ -303,9 +304,13 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     if (c->chunked) {
         cudaError_t e = cudaMalloc((void **)&c->dW, sizeof(double) * 4 * CH_MAX_P);
         if (e == cudaSuccess) e = cudaMemcpy(c->dW, c->fac.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&c->dS2, sizeof(double) * 144);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dS2, c->fac.Mlane, sizeof(double) * 128, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dS2 + 128, c->fac.WG, sizeof(double) * 16, cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
             std::string msg = std::string("ch_create: ") + cudaGetErrorString(e);
             if (c->dW) cudaFree(c->dW);
+            if (c->dS2) cudaFree(c->dS2);
             delete c;
             return fail(nullptr, e == cudaErrorMemoryAllocation ? CH_ENOMEM : CH_ECUDA, msg);
         }
@@ -365,6 +370,7 @@ extern "C" int ch_destroy(ch_ctx *ctx)
     if (ctx->ws_owned && ctx->ws_base) cudaFree(ctx->ws_base);
     if (ctx->dW) cudaFree(ctx->dW);
     if (ctx->dW16) cudaFree(ctx->dW16);
+    if (ctx->dS2) cudaFree(ctx->dS2);
     delete ctx;
     return CH_OK;
 }
@@ -564,8 +570,12 @@ static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
     memcpy(p.beta, c->fac.beta, sizeof(p.beta));
     p.W = c->dW; p.K = c->fac.K; p.P = c->fac.P;
     // log-depth closure (contiguous-line kernels only): worth it once the K-term sum is long
-    p.scan = 0;
+    p.scan = 0; p.scan2 = 0; p.S2 = c->dS2;
     const int P = c->fac.P;
+    if (c->opt_scan != 1 && (c->fac.K > 4 || c->opt_scan == 2) && P % 32 == 0 && P / 32 >= 2 && P / 32 <= 4) {
+        p.scan2 = P / 32;
+        memcpy(p.Mp, c->fac.Mpow2, sizeof(p.Mp));
+    }
     if (c->opt_scan != 1 && (c->fac.K > 4 || c->opt_scan == 2) && P >= 2 && P <= 32 && (P & (P - 1)) == 0) {
         int lg = 0;
         while ((1 << lg) < P) ++lg;
@@ -779,7 +789,7 @@ static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
     if (fuse_mode(c) == 4 && c->dW16) {
         memcpy(prm.alpha, c->fac16.alpha, sizeof(prm.alpha));
         memcpy(prm.beta, c->fac16.beta, sizeof(prm.beta));
-        prm.W = c->dW16; prm.K = c->fac16.K; prm.P = c->fac16.P; prm.scan = 0;
+        prm.W = c->dW16; prm.K = c->fac16.K; prm.P = c->fac16.P; prm.scan = 0; prm.scan2 = 0;
         LC = LINE_LC;
     }
     const int N = c->N, P = prm.P;

@@ -102,6 +102,16 @@ int ch_factor_build(ChFactor *f, int N, double sigma, int LC)
         for (int j = 0; j < f->P; ++j) MP = mul(MP, M);
         const M2 wc = inv_i_minus(MP);
         f->Wclose[0] = (double)wc.a; f->Wclose[1] = (double)wc.b; f->Wclose[2] = (double)wc.c; f->Wclose[3] = (double)wc.d;
+        M2 pj = { 1, 0, 0, 1 };
+        for (int j = 0; j < 32; ++j) {
+            f->Mlane[j][0] = (double)pj.a; f->Mlane[j][1] = (double)pj.b; f->Mlane[j][2] = (double)pj.c; f->Mlane[j][3] = (double)pj.d;
+            pj = mul(pj, M);
+        }
+        M2 g = wc;                       // pj is now M^32
+        for (int q = 0; q < 4; ++q) {
+            f->WG[q][0] = (double)g.a; f->WG[q][1] = (double)g.b; f->WG[q][2] = (double)g.c; f->WG[q][3] = (double)g.d;
+            g = mul(pj, g);
+        }
     }
     M2 close = { 1, 0, 0, 1 };
     if (K == f->P) {

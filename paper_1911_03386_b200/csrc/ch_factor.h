@@ -34,6 +34,11 @@ struct ChFactor {
     // T_{k+1}(c) = T_k(c) + M^(2^k) T_k(c - 2^k) (cyclic), s_in(c) = (I - M^P)^-1 T_log2P(c - 1)
     double Mpow2[7][4];        // M^(2^k), k = 0..6, row-major 2x2
     double Wclose[4];          // (I - M^P)^-1
+    // two-level form for lines of P = 32 W chunks, W = 2..4 (one warp scans 32 chunks, W warp aggregates are combined):
+    // state entering chunk c = [sum_{j=1..lane} M^(j-1) out(c-j)] + M^lane S_w,  S_w = sum_{q=1..W} WG[q-1] A_{w-q},
+    // A_w = sum_{j<32} M^j out(32 w + 31 - j),  WG[q-1] = (M^32)^(q-1) (I - M^P)^-1
+    double Mlane[32][4];       // M^j, j = 0..31
+    double WG[4][4];
     // generic path (one thread per line): closure of the whole line, (I - T^N)^-1
     double Wline[4];
 };

@@ -270,7 +270,7 @@ __global__ void k_sweep_x_update(const __grid_constant__ SweepParams prm, const 
         double2 x = live ? sl[swz<LC>(gbase + k)] : make_double2(0.0, 0.0);
         v[2 * k] = x.x; v[2 * k + 1] = x.y;
     }
-    if (prm.scan) chunk_solve_scan<LC>(prm, v, c);
+    if (prm.scan || prm.scan2) chunk_solve_scan<LC>(prm, v, c, sa + l * P);
     else chunk_solve<LC>(prm, v, sa + l * P, sb + l * P, c, 1);
     if (live) {
 #pragma unroll

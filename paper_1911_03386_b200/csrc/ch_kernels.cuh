@@ -24,6 +24,8 @@ struct SweepParams {
     double Mp[5][4];            // M^(2^k)
     double Wc[4];               // (I - M^P)^-1
     int scan;                   // 0, or log2 P (P a power of two, 2 <= P <= 32)
+    int scan2;                  // 0, or W = P / 32 in 2..4: two-level scan (warp scan + W warp aggregates)
+    const double *S2;           // device: Mlane[32][4] then WG[4][4] (ch_factor.h)
 };
 
 // 16-byte asynchronous global -> shared copy (L2 only), and its group fences
@@ -270,23 +272,67 @@ __device__ __forceinline__ void chunk_state_scan(const SweepParams &prm, double 
     b = fma(prm.Wc[2], ua, prm.Wc[3] * ub);
 }
 
+// Two-level form for P = 32 W chunks per line (W = 2..4 warps per line): a non-cyclic scan inside each warp,
+// the W warp aggregates combined through shared memory (agg: 2 W doubles per line and direction), and the
+// state entering the warp propagated to its lanes with the M^lane table.  One __syncthreads.
+__device__ __forceinline__ void chunk_state_scan2(const SweepParams &prm, double oa, double ob, int c, int dir,
+                                                  double *agg, double &a, double &b)
+{
+    const int W = prm.scan2, lane = c & 31, wl = c >> 5;
+    const int pos = dir > 0 ? lane : 31 - lane;                   // chunks between this one and the warp's entry side
+    double ta = oa, tb = ob;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int d = 1 << k;
+        const int src = dir > 0 ? lane - d : lane + d;
+        const double ua = __shfl_sync(0xffffffffu, ta, src & 31), ub = __shfl_sync(0xffffffffu, tb, src & 31);
+        if (pos >= d) {
+            ta = fma(prm.Mp[k][0], ua, fma(prm.Mp[k][1], ub, ta));
+            tb = fma(prm.Mp[k][2], ua, fma(prm.Mp[k][3], ub, tb));
+        }
+    }
+    if (pos == 31) { agg[2 * wl] = ta; agg[2 * wl + 1] = tb; }     // the warp's aggregate out-state
+    // exclusive part: what the chunks before this one (inside the warp) contribute
+    const int prev = dir > 0 ? lane - 1 : lane + 1;
+    double ea = __shfl_sync(0xffffffffu, ta, prev & 31), eb = __shfl_sync(0xffffffffu, tb, prev & 31);
+    if (pos == 0) { ea = 0.0; eb = 0.0; }
+    __syncthreads();
+    double sa_ = 0.0, sb_ = 0.0;
+    int w = wl;
+    for (int q = 0; q < W; ++q) {
+        w -= dir;
+        if (w < 0) w += W;
+        if (w >= W) w -= W;
+        const double ga = agg[2 * w], gb = agg[2 * w + 1];
+        const double *G = prm.S2 + 128 + 4 * q;
+        sa_ = fma(__ldg(G), ga, fma(__ldg(G + 1), gb, sa_));
+        sb_ = fma(__ldg(G + 2), ga, fma(__ldg(G + 3), gb, sb_));
+    }
+    const double2 m01 = __ldg(reinterpret_cast<const double2 *>(prm.S2) + 2 * pos);
+    const double2 m23 = __ldg(reinterpret_cast<const double2 *>(prm.S2) + 2 * pos + 1);
+    a = fma(m01.x, sa_, fma(m01.y, sb_, ea));
+    b = fma(m23.x, sa_, fma(m23.y, sb_, eb));
+}
+
 // Same solve as chunk_solve for kernels whose thread index is line * P + chunk (contiguous lines):
 // closure by warp-shuffle scan, no shared memory and no barrier.
 template <int LC>
-__device__ __forceinline__ void chunk_solve_scan(const SweepParams &prm, double (&v)[LC], int c)
+__device__ __forceinline__ void chunk_solve_scan(const SweepParams &prm, double (&v)[LC], int c, double *agg)
 {
     const double np = prm.np, nq = prm.nq;
     double a, b;
     v[1] = fma(np, v[0], v[1]);
 #pragma unroll
     for (int k = 2; k < LC; ++k) v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k]));
-    chunk_state_scan(prm, v[LC - 1], v[LC - 2], c, +1, a, b);
+    if (prm.scan2) chunk_state_scan2(prm, v[LC - 1], v[LC - 2], c, +1, agg, a, b);
+    else chunk_state_scan(prm, v[LC - 1], v[LC - 2], c, +1, a, b);
 #pragma unroll
     for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
     v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
 #pragma unroll
     for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
-    chunk_state_scan(prm, v[0], v[1], c, -1, a, b);
+    if (prm.scan2) chunk_state_scan2(prm, v[0], v[1], c, -1, agg + 8, a, b);
+    else chunk_state_scan(prm, v[0], v[1], c, -1, a, b);
 #pragma unroll
     for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
 }
@@ -395,7 +441,7 @@ __global__ void k_sweep_contig(const __grid_constant__ SweepParams prm, double *
         double2 x = live ? sl[swz<LC>(gbase + k)] : make_double2(0.0, 0.0);
         v[2 * k] = x.x; v[2 * k + 1] = x.y;
     }
-    if (prm.scan) chunk_solve_scan<LC>(prm, v, c);
+    if (prm.scan || prm.scan2) chunk_solve_scan<LC>(prm, v, c, sa + l * P);      // (sa, sb are contiguous: 2 P doubles per line pair)
     else chunk_solve<LC>(prm, v, sa + l * P, sb + l * P, c, 1);
     if (live) {
 #pragma unroll
