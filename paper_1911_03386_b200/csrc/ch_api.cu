@@ -34,6 +34,8 @@ struct ch_ctx {
     int LC;
     double *dW;             // device copy of fac.W
     double *dS2;            // device copy of fac.Mlane, fac.WG (two-level scan closure)
+    double *dS2_16;         // device copy of fac16.Mlane, fac16.WG
+    double *dS2c;           // cluster line SCAN kernels: fac16.Mlane then WG[8][4] of the cluster
     double *dW16;           // device copy of fac16.W (cluster line mode when c->LC is 32), else NULL
     double rscale;          // dt / c0^D: the 1/c0 of every sweep folded into the RHS
     // device arrays
@@ -236,7 +238,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         return fail(nullptr, CH_EINVAL, "ch_create: factorisation of I + gamma dt (delta^2)^2 failed its self-check");
     }
     c->rscale = dt / std::pow(c->fac.c0, D);
-    c->dW = nullptr; c->dW16 = nullptr; c->dS2 = nullptr;
+    c->dW = nullptr; c->dW16 = nullptr; c->dS2 = nullptr; c->dS2c = nullptr; c->dS2_16 = nullptr;
     c->nparts = rhs_parts(N, D);
     if (D == 2) { c->rhs_tiles_x = (N + RHS2_TX - 1) / RHS2_TX; c->rhs_tiles_y = (N + RHS2_TY - 1) / RHS2_TY; }
     else { c->rhs_tiles_x = (N + RHS3_TX - 1) / RHS3_TX; c->rhs_tiles_y = (N + RHS3_TY - 1) / RHS3_TY; }
@@ -249,8 +251,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
     c->cline_ok = false; c->cl_CS = 0; c->cl_strips = 0; c->cl_resident = 0;
     // (the chunk tables of a truncated closure do not depend on N: build them at a line length ch_factor allows)
-    if (D == 2 && (N == 1024 || N == 2048 || N == 4096) && ch_factor_build(&c->fac16, N < 2048 ? N : 2048, gamma * dt, LINE_LC) == 0
-        && c->fac16.K <= 2) {
+    if (D == 2 && (N == 1024 || N == 2048 || N == 4096) && ch_factor_build(&c->fac16, N < 2048 ? N : 2048, gamma * dt, LINE_LC) == 0) {
         c->cl_CS = N / CLINE_NC; c->cl_strips = (N + LINE_VALID - 1) / LINE_VALID;
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
@@ -259,23 +260,39 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         cfg.gridDim = dim3(c->cl_CS * 64); cfg.blockDim = dim3(CLINE_NC); cfg.dynamicSmemBytes = cline_smem();
         cfg.attrs = at; cfg.numAttrs = 1;
         int ncl = 0;
-        cudaError_t e;
-        if (c->cl_CS == 2) {
-            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<2>, &cfg);
-        } else if (c->cl_CS == 4) {
-            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<4>, &cfg);
-        } else {
-            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem());
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<8>, &cfg);
+        cudaError_t e = cudaSuccess;
+#define X(CSV)                                                                                                               \
+        if (c->cl_CS == CSV) {                                                                                                \
+            e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<CSV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem()); \
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_cline<CSV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cline_smem()); \
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&ncl, k_rhs_sweep_y_cline<CSV, true>, &cfg);           \
         }
+        X(2) X(4) X(8)
+#undef X
         if (e == cudaSuccess && ncl >= 1) { c->cline_ok = true; c->cl_resident = ncl; }
+        if (c->cline_ok && c->fac16.K > 2) {
+            // long closure: tables of the scan kernels (M^lane of a 16-point chunk, group closure of the cluster)
+            double tab[128 + 32];
+            double WG[8][4];
+            memcpy(tab, c->fac16.Mlane, sizeof(double) * 128);
+            if (ch_factor_groups(&c->fac16, c->cl_CS, WG) != 0) c->cline_ok = false;
+            memcpy(tab + 128, WG, sizeof(double) * 32);
+            if (c->cline_ok) e = cudaMalloc((void **)&c->dS2c, sizeof(tab));
+            if (c->cline_ok && e == cudaSuccess) e = cudaMemcpy(c->dS2c, tab, sizeof(tab), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) c->cline_ok = false;
+        }
         if (c->cline_ok && c->LC != LINE_LC && N / LINE_LC <= CH_MAX_P) {
             // the x-sweep of the cluster line step also runs at chunk length 16 (69 registers instead of 123)
             e = cudaMalloc((void **)&c->dW16, sizeof(double) * 4 * CH_MAX_P);
             if (e == cudaSuccess) e = cudaMemcpy(c->dW16, c->fac16.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
-            if (e != cudaSuccess) { if (c->dW16) cudaFree(c->dW16); c->dW16 = nullptr; }
+            if (e == cudaSuccess) e = cudaMalloc((void **)&c->dS2_16, sizeof(double) * 144);
+            if (e == cudaSuccess) e = cudaMemcpy(c->dS2_16, c->fac16.Mlane, sizeof(double) * 128, cudaMemcpyHostToDevice);
+            if (e == cudaSuccess) e = cudaMemcpy(c->dS2_16 + 128, c->fac16.WG, sizeof(double) * 16, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) {
+                if (c->dW16) cudaFree(c->dW16);
+                if (c->dS2_16) cudaFree(c->dS2_16);
+                c->dW16 = nullptr; c->dS2_16 = nullptr;
+            }
         }
         cudaGetLastError();
     }
@@ -371,6 +388,8 @@ extern "C" int ch_destroy(ch_ctx *ctx)
     if (ctx->dW) cudaFree(ctx->dW);
     if (ctx->dW16) cudaFree(ctx->dW16);
     if (ctx->dS2) cudaFree(ctx->dS2);
+    if (ctx->dS2c) cudaFree(ctx->dS2c);
+    if (ctx->dS2_16) cudaFree(ctx->dS2_16);
     delete ctx;
     return CH_OK;
 }
@@ -495,7 +514,7 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
     }
     if (!strcmp(key, "fuse")) {
         if (value < 0 || value > 4) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line) or 4 (cluster line)");
-        if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2, N in {1024, 2048, 4096} and a closure truncated to 2 chunks");
+        if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2 and N in {1024, 2048, 4096}");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
         if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 192, 256, 384, 512}");
         ctx->opt_fuse = value;
@@ -726,7 +745,9 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
     memcpy(p.beta, f.beta, sizeof(p.beta));
     memcpy(p.W0, f.W[0], sizeof(p.W0));
     memcpy(p.W1, f.W[1], sizeof(p.W1));
-    p.W = nullptr; p.K = f.K; p.scan = 0;
+    p.W = nullptr; p.K = f.K; p.scan = 0; p.S2 = c->dS2c;
+    memcpy(p.Mp, f.Mpow2, sizeof(p.Mp));
+    const bool scan = f.K > 2;
     p.ntiles = c->cl_strips * c->M; p.write = 1;
     const int ncl = p.ntiles < c->cl_resident ? p.ntiles : c->cl_resident;
     cudaLaunchConfig_t cfg = {};
@@ -735,9 +756,13 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
     at[0].val.clusterDim.x = c->cl_CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.gridDim = dim3(c->cl_CS * ncl); cfg.blockDim = dim3(CLINE_NC); cfg.dynamicSmemBytes = cline_smem();
     cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = 1;
-    if (c->cl_CS == 2) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<2>, p, (const double *)c->C, c->w);
-    else if (c->cl_CS == 4) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<4>, p, (const double *)c->C, c->w);
-    else cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<8>, p, (const double *)c->C, c->w);
+#define X(CSV)                                                                                                     \
+    if (c->cl_CS == CSV) {                                                                                          \
+        if (scan) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<CSV, true>, p, (const double *)c->C, c->w);          \
+        else cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<CSV, false>, p, (const double *)c->C, c->w);              \
+    }
+    X(2) X(4) X(8)
+#undef X
 }
 
 // number of F/Fdot/mass partials per member the fused RHS kernel in use writes
@@ -790,6 +815,10 @@ static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
         memcpy(prm.alpha, c->fac16.alpha, sizeof(prm.alpha));
         memcpy(prm.beta, c->fac16.beta, sizeof(prm.beta));
         prm.W = c->dW16; prm.K = c->fac16.K; prm.P = c->fac16.P; prm.scan = 0; prm.scan2 = 0;
+        if (c->opt_scan != 1 && (prm.K > 4 || c->opt_scan == 2) && prm.P % 32 == 0 && prm.P / 32 >= 2 && prm.P / 32 <= 4) {
+            prm.scan2 = prm.P / 32; prm.S2 = c->dS2_16;
+            memcpy(prm.Mp, c->fac16.Mpow2, sizeof(prm.Mp));
+        }
         LC = LINE_LC;
     }
     const int N = c->N, P = prm.P;

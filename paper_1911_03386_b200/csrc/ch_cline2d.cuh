@@ -55,9 +55,11 @@ __device__ __forceinline__ void cl_sync_all()
 // (the last two are ghosts written by the next CTA).
 #define CLINE_NC 512
 #define CLINE_P (CLINE_NC / LINE_LC)
-#define CLINE_SLOT ((CLINE_P + 2) * 16)
+#define CLINE_SS 17                              /* lane stride of a chunk's slots in the SCAN kernels (conflict-free transposed access) */
+#define CLINE_SLOT ((CLINE_P + 2) * CLINE_SS)
 
-static inline size_t cline_smem() { return (size_t)(LINE_LC + 4) * CLINE_NC * 16 + (size_t)4 * CLINE_SLOT * 16; }
+#define CH_MAX_CS 8
+static inline size_t cline_smem() { return (size_t)(LINE_LC + 4) * CLINE_NC * 16 + (size_t)4 * CLINE_SLOT * 16 + (size_t)2 * CH_MAX_CS * 32 * 16; }
 
 // first: index of the nearer of the two chunks (c - 1 + 2 forward, c + 1 backward); step: -1 / +1
 __device__ __forceinline__ void cline_state_in(const LineParams &prm, const double2 *slots, int first, int step, int li,
@@ -78,14 +80,79 @@ __device__ __forceinline__ void cline_state_in(const LineParams &prm, const doub
     }
 }
 
-// grid = CS * min(ntiles, resident clusters) with cluster dimension CS, block = 512,
-// dynamic smem = cline_smem().  Requires prm.K <= 2.
+// Closure for long K (SCAN kernels; paper-regime gamma dt): called by every thread after its chunk states
+// are in `slots` ([column A|B][P + 2 chunks][16 lanes], this direction's local chunks at index base + c).
+//  1. CTA barrier; the slots are re-read transposed (lane = chunk, one column per warp pass, two passes) and
+//     scanned NON-cyclically with shuffles: T(c) = sum_{j <= pos} M^j out(c -+ j), pos = chunks since the CTA's
+//     entry side; the exclusive part goes back into the slot, the CTA aggregate T(pos = 31) is pushed into
+//     agg[rank][column] of EVERY CTA of the cluster (remote shared-memory stores);
+//  2. cluster barrier (release/acquire: the pushes are visible, and it is a CTA barrier too);
+//  3. state entering chunk c = exclusive(c) + M^pos S,  S = sum_{q=1..CS} WG[q-1] A_{rank -+ q}
+//     (ch_factor.h, two-level form; tables prm.S2 = Mlane[32][4] then WG[8][4] in device memory).
 template <int CS>
+__device__ __forceinline__ void cline_scan_closure(const LineParams &prm, double2 *slots, int base, double2 *agg, int tid,
+                                                   unsigned rank, int dir, double &aA, double &bA, double &aB, double &bB)
+{
+    constexpr int P = CLINE_P;
+    const int lane = tid & 31, wid = tid >> 5, li = tid & 15, c = tid >> 4;
+    __syncthreads();
+    const int pos_l = dir > 0 ? lane : 31 - lane;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const int col = q * 16 + wid;                                 // 0..31: [column A|B][16 lanes]
+        double2 *slot = slots + (col >> 4) * CLINE_SLOT + (base + lane) * CLINE_SS + (col & 15);
+        const double2 o = *slot;
+        double ta = o.x, tb = o.y;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const int d = 1 << k, src = dir > 0 ? lane - d : lane + d;
+            const double ua = __shfl_sync(0xffffffffu, ta, src & 31), ub = __shfl_sync(0xffffffffu, tb, src & 31);
+            if (pos_l >= d) {
+                ta = fma(prm.Mp[k][0], ua, fma(prm.Mp[k][1], ub, ta));
+                tb = fma(prm.Mp[k][2], ua, fma(prm.Mp[k][3], ub, tb));
+            }
+        }
+        const int prev = dir > 0 ? lane - 1 : lane + 1;
+        double ea = __shfl_sync(0xffffffffu, ta, prev & 31), eb = __shfl_sync(0xffffffffu, tb, prev & 31);
+        if (pos_l == 0) { ea = 0.0; eb = 0.0; }
+        *slot = make_double2(ea, eb);
+        if (pos_l == 31) {
+            const double2 A = make_double2(ta, tb);
+#pragma unroll 1
+            for (unsigned rk = 0; rk < CS; ++rk) cl_store2(cl_map(agg + rank * 32 + col, rk), A);
+        }
+    }
+    cl_sync_all();
+    double SaA = 0.0, SbA = 0.0, SaB = 0.0, SbB = 0.0;
+    int r = (int)rank;
+#pragma unroll 1
+    for (int q = 0; q < CS; ++q) {
+        r -= dir;
+        if (r < 0) r += CS;
+        if (r >= CS) r -= CS;
+        const double2 gA = agg[r * 32 + li], gB = agg[r * 32 + 16 + li];
+        const double2 w01 = __ldg(reinterpret_cast<const double2 *>(prm.S2) + 64 + 2 * q);
+        const double2 w23 = __ldg(reinterpret_cast<const double2 *>(prm.S2) + 64 + 2 * q + 1);
+        SaA = fma(w01.x, gA.x, fma(w01.y, gA.y, SaA)); SbA = fma(w23.x, gA.x, fma(w23.y, gA.y, SbA));
+        SaB = fma(w01.x, gB.x, fma(w01.y, gB.y, SaB)); SbB = fma(w23.x, gB.x, fma(w23.y, gB.y, SbB));
+    }
+    const int pos = dir > 0 ? c : P - 1 - c;
+    const double2 m01 = __ldg(reinterpret_cast<const double2 *>(prm.S2) + 2 * pos);
+    const double2 m23 = __ldg(reinterpret_cast<const double2 *>(prm.S2) + 2 * pos + 1);
+    const double2 eA = slots[(base + c) * CLINE_SS + li], eB = slots[CLINE_SLOT + (base + c) * CLINE_SS + li];
+    aA = fma(m01.x, SaA, fma(m01.y, SbA, eA.x)); bA = fma(m23.x, SaA, fma(m23.y, SbA, eA.y));
+    aB = fma(m01.x, SaB, fma(m01.y, SbB, eB.x)); bB = fma(m23.x, SaB, fma(m23.y, SbB, eB.y));
+}
+
+// grid = CS * min(ntiles, resident clusters) with cluster dimension CS, block = 512,
+// dynamic smem = cline_smem().  SCAN == false requires prm.K <= 2 (neighbour flags); SCAN == true handles any K.
+template <int CS, bool SCAN>
 __global__ void __launch_bounds__(CLINE_NC, 1) k_rhs_sweep_y_cline(const __grid_constant__ LineParams prm,
                                                                   const double *__restrict__ C, double *__restrict__ w)
 {
     constexpr int LC = LINE_LC, NR = LC + 4, NT = CLINE_NC, P = CLINE_P, N = CLINE_NC * CS, NW = NT / 32;
     constexpr int strips = (N + LINE_VALID - 1) / LINE_VALID;
+    constexpr int SS = SCAN ? CLINE_SS : 16;
     constexpr size_t n2 = (size_t)N * N;
     extern __shared__ double2 sm2[];
     __shared__ unsigned flagF[NW], flagB[NW], gflagF, gflagB;
@@ -95,6 +162,7 @@ __global__ void __launch_bounds__(CLINE_NC, 1) k_rhs_sweep_y_cline(const __grid_
     const int cg = (int)rank * P + c;                              // chunk index along the whole line
     double2 *stage = sm2 + tid;
     double2 *slotF = sm2 + (size_t)NR * NT, *slotB = slotF + 2 * CLINE_SLOT;
+    double2 *aggF = slotB + 2 * CLINE_SLOT, *aggB = aggF + CH_MAX_CS * 32;      // SCAN: CTA aggregates [rank][32 columns]
     if (tid < NW) { flagF[tid] = 0; flagB[tid] = 0; }
     if (tid == 0) { gflagF = 0; gflagB = 0; }
     __syncthreads();
@@ -178,18 +246,22 @@ __global__ void __launch_bounds__(CLINE_NC, 1) k_rhs_sweep_y_cline(const __grid_
         ++seq;
         {
             const double2 sA = make_double2(vA[LC - 1], vA[LC - 2]), sB = make_double2(vB[LC - 1], vB[LC - 2]);
-            slotF[(c + 2) * 16 + li] = sA;
-            slotF[CLINE_SLOT + (c + 2) * 16 + li] = sB;
-            if (wid == NW - 1) { cl_store2(remSlot, sA); cl_store2(remSlot + CLINE_SLOT * 16, sB); }
-            __syncwarp();
-            if ((tid & 31) == 0) {
-                flag_release(&flagF[wid], seq);
-                if (wid == NW - 1) cl_flag_release(remFlag, seq);
-            }
-            if (wid == 0) cl_flag_wait(&gflagF, seq); else flag_wait(&flagF[wid - 1], seq);
-            __syncwarp();
+            slotF[(c + 2) * SS + li] = sA;
+            slotF[CLINE_SLOT + (c + 2) * SS + li] = sB;
             double aA, bA, aB, bB;
-            cline_state_in(prm, slotF, c + 1, -1, li, aA, bA, aB, bB);
+            if (SCAN) {
+                cline_scan_closure<CS>(prm, slotF, 2, aggF, tid, rank, +1, aA, bA, aB, bB);
+            } else {
+                if (wid == NW - 1) { cl_store2(remSlot, sA); cl_store2(remSlot + CLINE_SLOT * 16, sB); }
+                __syncwarp();
+                if ((tid & 31) == 0) {
+                    flag_release(&flagF[wid], seq);
+                    if (wid == NW - 1) cl_flag_release(remFlag, seq);
+                }
+                if (wid == 0) cl_flag_wait(&gflagF, seq); else flag_wait(&flagF[wid - 1], seq);
+                __syncwarp();
+                cline_state_in(prm, slotF, c + 1, -1, li, aA, bA, aB, bB);
+            }
 #pragma unroll
             for (int k = 0; k < LC; ++k) {
                 vA[k] = fma(prm.alpha[k], aA, fma(prm.beta[k], bA, vA[k]));
@@ -206,18 +278,22 @@ __global__ void __launch_bounds__(CLINE_NC, 1) k_rhs_sweep_y_cline(const __grid_
         }
         {
             const double2 sA = make_double2(vA[0], vA[1]), sB = make_double2(vB[0], vB[1]);
-            slotB[c * 16 + li] = sA;
-            slotB[CLINE_SLOT + c * 16 + li] = sB;
-            if (wid == 0) { cl_store2(remSlot, sA); cl_store2(remSlot + CLINE_SLOT * 16, sB); }
-            __syncwarp();
-            if ((tid & 31) == 0) {
-                flag_release(&flagB[wid], seq);
-                if (wid == 0) cl_flag_release(remFlag, seq);
-            }
-            if (wid == NW - 1) cl_flag_wait(&gflagB, seq); else flag_wait(&flagB[wid + 1], seq);
-            __syncwarp();
+            slotB[c * SS + li] = sA;
+            slotB[CLINE_SLOT + c * SS + li] = sB;
             double aA, bA, aB, bB;
-            cline_state_in(prm, slotB, c + 1, +1, li, aA, bA, aB, bB);
+            if (SCAN) {
+                cline_scan_closure<CS>(prm, slotB, 0, aggB, tid, rank, -1, aA, bA, aB, bB);
+            } else {
+                if (wid == 0) { cl_store2(remSlot, sA); cl_store2(remSlot + CLINE_SLOT * 16, sB); }
+                __syncwarp();
+                if ((tid & 31) == 0) {
+                    flag_release(&flagB[wid], seq);
+                    if (wid == 0) cl_flag_release(remFlag, seq);
+                }
+                if (wid == NW - 1) cl_flag_wait(&gflagB, seq); else flag_wait(&flagB[wid + 1], seq);
+                __syncwarp();
+                cline_state_in(prm, slotB, c + 1, +1, li, aA, bA, aB, bB);
+            }
             const int t2 = opaque(tile), tid2 = opaque(tid);
             const int strip2 = t2 % strips, m2 = t2 / strips, li2 = tid2 & 15;
             const int gx = strip2 * LINE_VALID - 2 + 2 * li2;

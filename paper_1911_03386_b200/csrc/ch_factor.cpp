@@ -126,3 +126,19 @@ int ch_factor_build(ChFactor *f, int N, double sigma, int LC)
     }
     return 0;
 }
+
+int ch_factor_groups(const ChFactor *f, int groups, double WG[8][4])
+{
+    if (f->LC < 2 || groups < 1 || groups > 8) return -1;
+    const M2 M = transfer((ld)f->np, (ld)f->nq, f->LC, nullptr, nullptr);
+    M2 M32 = { 1, 0, 0, 1 };
+    for (int j = 0; j < 32; ++j) M32 = mul(M32, M);
+    M2 MP = { 1, 0, 0, 1 };
+    for (int j = 0; j < groups; ++j) MP = mul(MP, M32);
+    M2 g = inv_i_minus(MP);
+    for (int q = 0; q < 8; ++q) {
+        WG[q][0] = (double)g.a; WG[q][1] = (double)g.b; WG[q][2] = (double)g.c; WG[q][3] = (double)g.d;
+        g = mul(M32, g);
+    }
+    return 0;
+}

@@ -46,3 +46,7 @@ struct ChFactor {
 // Fill f for line length N and chunk length LC (LC == 0: generic path only).
 // Returns 0, or -1 if the factorisation failed its self-check.
 int ch_factor_build(ChFactor *f, int N, double sigma, int LC);
+
+// WG[q] = (M^32)^q (I - (M^32)^groups)^-1, q = 0..7, for a line of `groups` groups of 32 chunks of f->LC points
+// (the two-level closure across the CTAs of a cluster, ch_cline2d.cuh).  Returns 0, or -1 on bad arguments.
+int ch_factor_groups(const ChFactor *f, int groups, double WG[8][4]);

@@ -34,6 +34,7 @@ struct LineParams {
     // log-depth closure of the barrier kernels when the K-term sum is long (ch_factor.h, Mpow2 / Wclose)
     double Mp[5][4], Wc[4];
     int scan;                       // 0, or log2 P (P a power of two)
+    const double *S2;               // cluster line SCAN kernels: device Mlane[32][4] then WG[8][4] (ch_factor.h)
 };
 
 __device__ __forceinline__ void line_cp_async16(void *smem_dst, const void *gsrc)

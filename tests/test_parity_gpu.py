@@ -282,7 +282,7 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     e.close()
     assert (cs == 0) == (N == 592)
     assert (line != 0) == (N in (32, 64, 96, 128, 192, 256, 384, 512))
-    assert (cline != 0) == (N == 1024 and gamma == 1.0)        # K <= 2 only: not in the paper regime
+    assert (cline != 0) == (N == 1024)                         # flag kernel at K <= 2, scan kernel in the paper regime
     assert mode == (3 if line else (4 if cline else (2 if cs else 0)))
     variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
         + ([{"fuse": 4}] if cline else [])
