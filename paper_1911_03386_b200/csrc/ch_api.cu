@@ -175,7 +175,7 @@ static bool rhs3_stream_geometry(int N, int D, int *parts)
 static size_t line_smem(int N)
 {
     const int P = N / LINE_LC;
-    return (size_t)(LINE_LC + 4) * 16 * P * 16 + (size_t)4 * P * 16 * 16;
+    return (size_t)(LINE_LC + 4) * 16 * P * 16 + (size_t)4 * P * LINE_SS * 16;
 }
 
 static int max_parts(int N, int D)

@@ -22,6 +22,7 @@
 
 #define LINE_LC 16
 #define LINE_VALID 28         // columns a half-warp produces: 16 lanes x 2 columns minus a halo of 2 on either side
+#define LINE_SS 17            // lane stride of the slots in the barrier kernels (conflict-free transposed re-read)
 #define LINE_MAX_P 32         // chunks per line: 16 * P threads per CTA
 
 struct LineParams {
@@ -72,14 +73,14 @@ __device__ __forceinline__ int opaque(int x) { asm volatile("" : "+r"(x)); retur
 
 // states entering chunk c (both columns of the lane) from the K chunks before it (dir = +1) or after
 // it (dir = -1); slots are [column A|B][chunk][16 lanes] pairs (value next to the boundary, one further in)
-template <int P>
+template <int P, int SS>
 __device__ __forceinline__ void line_state_in(const LineParams &prm, const double2 *slots, int tid, int dir,
                                               double &aA, double &bA, double &aB, double &bB)
 {
     const int c = tid >> 4, li = tid & 15;
     aA = bA = aB = bB = 0.0;
     auto acc = [&](int s, double w0, double w1, double w2, double w3) {
-        const double2 oA = slots[s * 16 + li], oB = slots[(P + s) * 16 + li];
+        const double2 oA = slots[s * SS + li], oB = slots[(P + s) * SS + li];
         aA = fma(w0, oA.x, fma(w1, oA.y, aA));
         bA = fma(w2, oA.x, fma(w3, oA.y, bA));
         aB = fma(w0, oB.x, fma(w1, oB.y, aB));
@@ -104,7 +105,7 @@ __device__ __forceinline__ void line_state_in(const LineParams &prm, const doubl
 // slots are re-read TRANSPOSED -- lane = chunk, 32 / P columns per warp pass, two passes cover the 32
 // columns -- scanned with width-P shuffles exactly as chunk_state_scan (ch_kernels.cuh), written back in
 // place as the states ENTERING each chunk, and after one more barrier every thread picks up its own.
-template <int P>
+template <int P, int SS>
 __device__ __forceinline__ void line_scan_closure(const LineParams &prm, double2 *slots, int tid, int dir,
                                                   double &aA, double &bA, double &aB, double &bB)
 {
@@ -113,7 +114,7 @@ __device__ __forceinline__ void line_scan_closure(const LineParams &prm, double2
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
         const int col = q * 16 + wid * CPW + lane / P;
-        double2 *slot = slots + ((col >> 4) * P + ch) * 16 + (col & 15);
+        double2 *slot = slots + ((col >> 4) * P + ch) * SS + (col & 15);
         const double2 o = *slot;
         double ta = o.x, tb = o.y;
         for (int k = 0; k < prm.scan; ++k) {
@@ -127,7 +128,7 @@ __device__ __forceinline__ void line_scan_closure(const LineParams &prm, double2
         *slot = make_double2(fma(prm.Wc[0], ua, prm.Wc[1] * ub), fma(prm.Wc[2], ua, prm.Wc[3] * ub));
     }
     __syncthreads();
-    const double2 sA = slots[tid], sB = slots[16 * P + tid];
+    const double2 sA = slots[(tid >> 4) * SS + (tid & 15)], sB = slots[(P + (tid >> 4)) * SS + (tid & 15)];
     aA = sA.x; bA = sA.y; aB = sB.x; bB = sB.y;
 }
 
@@ -160,7 +161,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
     const bool lane_ok = li >= 1 && li < 15;
 
     double2 *stage = sm2 + tid;                                   // row j of this thread: stage[j * NT]
-    double2 *slotF = sm2 + (size_t)NR * NT, *slotB = slotF + 2 * P * 16;
+    constexpr int SS = NB ? 16 : LINE_SS;                       // lane stride of a chunk's slots
+    double2 *slotF = sm2 + (size_t)NR * NT, *slotB = slotF + 2 * P * LINE_SS;
 
     // C rows y0-2 .. y0+LC+1 of this thread's column pair; only the two halo rows on either end wrap
     auto tile_base = [&](int tile) {
@@ -259,8 +261,13 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
 
         // ---- forward closure
-        slotF[tid] = make_double2(vA[LC - 1], vA[LC - 2]);              // [column A|B][chunk][lane]: c * 16 + li == tid
-        slotF[NT + tid] = make_double2(vB[LC - 1], vB[LC - 2]);
+        if (NB) {                                                       // [column A|B][chunk][lane]: c * 16 + li == tid
+            slotF[tid] = make_double2(vA[LC - 1], vA[LC - 2]);
+            slotF[NT + tid] = make_double2(vB[LC - 1], vB[LC - 2]);
+        } else {
+            slotF[c * SS + li] = make_double2(vA[LC - 1], vA[LC - 2]);
+            slotF[(P + c) * SS + li] = make_double2(vB[LC - 1], vB[LC - 2]);
+        }
         ++seq;
         if (NB) {
             __syncwarp();
@@ -272,8 +279,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
         {
             double aA, bA, aB, bB;
-            if (!NB && (P & (P - 1)) == 0 && prm.scan) line_scan_closure<P>(prm, slotF, tid, +1, aA, bA, aB, bB);
-            else line_state_in<P>(prm, slotF, tid, +1, aA, bA, aB, bB);
+            if (!NB && (P & (P - 1)) == 0 && prm.scan) line_scan_closure<P, SS>(prm, slotF, tid, +1, aA, bA, aB, bB);
+            else line_state_in<P, SS>(prm, slotF, tid, +1, aA, bA, aB, bB);
 #pragma unroll
             for (int k = 0; k < LC; ++k) {
                 vA[k] = fma(prm.alpha[k], aA, fma(prm.beta[k], bA, vA[k]));
@@ -288,8 +295,13 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
             vA[k] = fma(np, vA[k + 1], fma(nq, vA[k + 2], vA[k]));
             vB[k] = fma(np, vB[k + 1], fma(nq, vB[k + 2], vB[k]));
         }
-        slotB[tid] = make_double2(vA[0], vA[1]);
-        slotB[NT + tid] = make_double2(vB[0], vB[1]);
+        if (NB) {
+            slotB[tid] = make_double2(vA[0], vA[1]);
+            slotB[NT + tid] = make_double2(vB[0], vB[1]);
+        } else {
+            slotB[c * SS + li] = make_double2(vA[0], vA[1]);
+            slotB[(P + c) * SS + li] = make_double2(vB[0], vB[1]);
+        }
         if (NB) {
             __syncwarp();
             if ((tid & 31) == 0) flag_release(&flagB[wid], seq);
@@ -300,8 +312,8 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         }
         {
             double aA, bA, aB, bB;
-            if (!NB && (P & (P - 1)) == 0 && prm.scan) line_scan_closure<P>(prm, slotB, tid, -1, aA, bA, aB, bB);
-            else line_state_in<P>(prm, slotB, tid, -1, aA, bA, aB, bB);
+            if (!NB && (P & (P - 1)) == 0 && prm.scan) line_scan_closure<P, SS>(prm, slotB, tid, -1, aA, bA, aB, bB);
+            else line_state_in<P, SS>(prm, slotB, tid, -1, aA, bA, aB, bB);
             // where this thread's results go, recomputed from the tile and thread index
             const int t2 = opaque(tile), tid2 = opaque(tid);
             const int strip2 = t2 % strips, m2 = t2 / strips, li2 = tid2 & 15;
