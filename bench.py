@@ -32,7 +32,7 @@ FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS
 ALGO_BYTES = {
     2: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 24,
         "rhs_sweep_y": 16, "rhs_sweep_y_diag": 16, "sweep_x_update": 24},      # fused 2D step: 40 B per update
-    3: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 16, "sweep_z": 24},
+    3: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 16, "sweep_z": 24, "sweep_xy": 16},   # plane kernel: x + y in one pass
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, kernel); None until captured.
@@ -228,7 +228,7 @@ def run_ours(args):
     # bytes one step must move in the pass structure that ran: fused 2D step 16 + 24 = 40 B per update
     # (DESIGN.md section 5), three-pass 2D 56 B, four-pass 3D 72 B
     fused = "sweep_x_update" in kernels
-    step_bytes = 40 if fused else (56 if D == 2 else 72)
+    step_bytes = 40 if fused else (56 if D == 2 else (56 if "sweep_xy" in kernels else 72))
     model_bytes = 56 if D == 2 else 72
     main_kinds = {k: v for k, v in kernels.items() if not k.endswith("_diag")} or kernels
     dom = max(main_kinds, key=lambda k: main_kinds[k]["avg_ms"] * main_kinds[k]["launches"])

@@ -135,7 +135,7 @@ int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
 /* Per-kernel device timing.  ch_profile(ctx, 1) makes every later launch be bracketed by CUDA
  * events on the context's stream; ch_profile_read synchronises, returns the summed milliseconds
  * and launch counts per kernel kind (ch_kernel_kinds() kinds, named by ch_kernel_kind_name:
- * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z, rhs_sweep_y, rhs_sweep_y_diag, sweep_x_update)
+ * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z, rhs_sweep_y, rhs_sweep_y_diag, sweep_x_update, sweep_xy)
  * and clears the records. */
 int ch_profile(ch_ctx *ctx, int enable);
 int ch_profile_read(ch_ctx *ctx, double *ms, long long *counts, int nkinds);

@@ -16,9 +16,9 @@
 #include "ch_cline2d.cuh"
 
 enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z,
-       KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_COUNT };
+       KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_SWEEP_XY, KIND_COUNT };
 static const char *const kKindNames[KIND_COUNT] = { "rhs", "rhs_diag", "finish", "sweep_x", "sweep_y", "sweep_z",
-                                                    "rhs_sweep_y", "rhs_sweep_y_diag", "sweep_x_update" };
+                                                    "rhs_sweep_y", "rhs_sweep_y_diag", "sweep_x_update", "sweep_xy" };
 
 struct ProfRec { int kind; cudaEvent_t e0, e1; };
 
@@ -69,6 +69,8 @@ struct ch_ctx {
     bool r3_ok;
     int r3_parts, r3_resident;   // partials per member, CTAs resident on the device
     int opt_rhs3;                // 0 auto (streaming kernel when available), 1 tile kernel
+    bool xy_ok;                  // 3D, N in {64, 128}: x- and y-sweep of a z-plane in one pass (k_sweep_xy_plane)
+    int opt_sweep3;              // 0 auto (plane kernel when available), 1 separate x and y sweeps
     // fused 2D step, whole line in one CTA (ch_line2d.cuh)
     bool line_ok;
     int l_strips, l_resident;    // column strips per member, CTAs resident on the device
@@ -296,6 +298,15 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         }
         cudaGetLastError();
     }
+    c->opt_sweep3 = 0;
+    c->xy_ok = D == 3 && (N == 64 || N == 128) && c->chunked;
+    if (c->xy_ok) {
+        const int smem = N * N * 8 + 2 * (N / 16) * N * 8;
+        cudaError_t e = N == 64 ? cudaFuncSetAttribute(k_sweep_xy_plane<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)
+                                : cudaFuncSetAttribute(k_sweep_xy_plane<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) c->xy_ok = false;
+        cudaGetLastError();
+    }
     c->r3_parts = 0; c->r3_resident = 0; c->opt_rhs3 = 0;
     c->r3_ok = rhs3_stream_geometry(N, D, &c->r3_parts);
     if (c->r3_ok) {
@@ -502,6 +513,11 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_scan = value;
         return CH_OK;
     }
+    if (!strcmp(key, "sweep3")) {
+        if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: sweep3 must be 0 (auto) or 1 (separate x and y sweeps)");
+        ctx->opt_sweep3 = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "rhs3")) {
         if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: rhs3 must be 0 (auto) or 1 (tile kernel)");
         ctx->opt_rhs3 = value;
@@ -531,6 +547,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
     if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
     if (!strcmp(key, "fused")) { *value = ctx->fused_ok ? ctx->f_CS : 0; return CH_OK; }
+    if (!strcmp(key, "sweep_xy")) { *value = (ctx->xy_ok && ctx->opt_sweep3 != 1 && ctx->opt_sweep != 1) ? 1 : 0; return CH_OK; }
     if (!strcmp(key, "rhs3_stream")) { *value = use_rhs3_stream(ctx) ? ctx->r3_resident : 0; return CH_OK; }
     if (!strcmp(key, "cline")) { *value = ctx->cline_ok ? ctx->cl_resident : 0; return CH_OK; }
     if (!strcmp(key, "line")) { *value = ctx->line_ok ? ctx->l_resident : 0; return CH_OK; }
@@ -684,6 +701,24 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
 }
 
 static bool use_fused(const ch_ctx *c) { return fuse_mode(c) != 0; }
+
+// 3D: x- and y-sweep of every z-plane in one pass
+static void launch_sweep_xy(ch_ctx *c, double *w)
+{
+    ProfScope ps(c, KIND_SWEEP_XY);
+    SweepParams prm;
+    fill_params(c, prm, 1.0);
+    const int P = c->fac.P;
+    prm.scan = 0; prm.scan2 = 0;
+    while ((1 << prm.scan) < P) ++prm.scan;
+    memcpy(prm.Mp, c->fac.Mpow2, sizeof(prm.Mp));
+    memcpy(prm.Wc, c->fac.Wclose, sizeof(prm.Wc));
+    const int N = c->N;
+    const size_t smem = (size_t)N * N * 8 + (size_t)2 * P * N * 8;
+    const unsigned planes = (unsigned)((size_t)c->M * N);
+    if (N == 64) k_sweep_xy_plane<64><<<planes, 256, smem, c->stream>>>(prm, w);
+    else k_sweep_xy_plane<128><<<planes, 1024, smem, c->stream>>>(prm, w);
+}
 
 // ---- fused 2D step: (RHS + y-sweep) then (x-sweep + update) ------------------------------------
 template <int LC, bool DIAG>
@@ -867,6 +902,10 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
             ctx->cursor++; ctx->last_sampled = ctx->n;
         }
         if (fused) launch_sweep_x_update(ctx, unscaled);
+        else if (D == 3 && ctx->xy_ok && ctx->opt_sweep3 != 1 && ctx->opt_sweep != 1) {
+            launch_sweep_xy(ctx, ctx->w);
+            launch_sweep(ctx, ctx->w, 2, true, false, 1.0);
+        }
         else for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
         ctx->n++;
     }

@@ -532,3 +532,52 @@ __global__ void __launch_bounds__(256) k_sweep_pcr_x(const __grid_constant__ Pcr
     }
     for (int i = threadIdx.x; i < N; i += 256) g[i] = cur[i] * prm.final_scale;
 }
+
+// ------------------------------------------------------------------------------------
+// 3D: x- and y-sweep of one z-plane in one pass (N = 64, 128: the plane, N^2 * 8 B <= 128 KB, lives in
+// shared memory), w := A_y^-1 A_x^-1 w.  Saves one full read + write of the field: 16 B per update
+// instead of 32 B.  CTA = one plane of one member, NC * NC / 16 threads.
+//   x phase: thread (row, chunk of 16 contiguous points), plane in the swizzled granule layout of
+//            k_sweep_contig, closure by width-P shuffle scan (the P = NC / 16 chunks of a row sit in
+//            consecutive lanes): no barrier;
+//   y phase: thread (column, chunk of 16 rows) reads its column from shared memory (a warp reads 32
+//            consecutive doubles of a row), chunk_solve with the exchange through shared memory,
+//            results written straight to global memory (coalesced rows).
+// dynamic smem = NC * NC * 8 + 2 * (NC / 16) * NC * 8.  prm.scan must be log2(NC / 16) with Mp, Wc filled.
+// ------------------------------------------------------------------------------------
+template <int NC>
+__global__ void __launch_bounds__(NC * NC / 16, NC == 64 ? 3 : 1) k_sweep_xy_plane(const __grid_constant__ SweepParams prm, double *__restrict__ w)
+{
+    constexpr int LC = 16, P = NC / LC, NT = NC * NC / LC, G = NC * NC / 2;
+    extern __shared__ double2 sl[];
+    double *sx = reinterpret_cast<double *>(sl + G);
+    const int t = threadIdx.x;
+    double2 *g2 = reinterpret_cast<double2 *>(w + (size_t)blockIdx.x * NC * NC);
+#pragma unroll
+    for (int k = 0; k < G / NT; ++k) ck_cp_async16(&sl[swz<LC>(k * NT + t)], g2 + k * NT + t);
+    ck_cp_async_wait_all();
+    __syncthreads();
+    double v[LC];
+    {   // x phase
+        const int l = t / P, c = t - l * P, gbase = l * (NC / 2) + c * (LC / 2);
+#pragma unroll
+        for (int k = 0; k < LC / 2; ++k) { const double2 x = sl[swz<LC>(gbase + k)]; v[2 * k] = x.x; v[2 * k + 1] = x.y; }
+        chunk_solve_scan<LC>(prm, v, c, nullptr);
+#pragma unroll
+        for (int k = 0; k < LC / 2; ++k) sl[swz<LC>(gbase + k)] = make_double2(v[2 * k], v[2 * k + 1]);
+    }
+    __syncthreads();
+    {   // y phase
+        const int x = t % NC, c = t / NC;
+        const double *sd = reinterpret_cast<const double *>(sl);
+#pragma unroll
+        for (int k = 0; k < LC; ++k) {
+            const int g = (c * LC + k) * (NC / 2) + (x >> 1);
+            v[k] = sd[2 * swz<LC>(g) + (x & 1)];
+        }
+        chunk_solve<LC>(prm, v, sx + x, sx + P * NC + x, c, NC);      // the strided closure sums K terms through shared memory
+        double *o = w + (size_t)blockIdx.x * NC * NC + (size_t)c * LC * NC + x;
+#pragma unroll
+        for (int k = 0; k < LC; ++k) o[k * NC] = v[k];
+    }
+}

@@ -52,9 +52,9 @@ def test_workspace_bytes_and_argument_errors(lib):
     assert b"ch_create" in lib.ch_last_error(None)
     assert lib.ch_destroy(None) == binding.CH_EINVAL
     assert lib.ch_step(None, 1) == binding.CH_EINVAL
-    assert lib.ch_kernel_kinds() == 9
-    assert [lib.ch_kernel_kind_name(k) for k in range(9)] == [b"rhs", b"rhs_diag", b"finish", b"sweep_x", b"sweep_y", b"sweep_z",
-                                                               b"rhs_sweep_y", b"rhs_sweep_y_diag", b"sweep_x_update"]
+    assert lib.ch_kernel_kinds() == 10
+    assert [lib.ch_kernel_kind_name(k) for k in range(10)] == [b"rhs", b"rhs_diag", b"finish", b"sweep_x", b"sweep_y", b"sweep_z",
+                                                                b"rhs_sweep_y", b"rhs_sweep_y_diag", b"sweep_x_update", b"sweep_xy"]
 
 
 def test_no_cpu_fallback_without_a_gpu(lib):

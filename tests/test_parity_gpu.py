@@ -187,10 +187,27 @@ def test_3d_streaming_and_tile_rhs(B, oracle):
     Ct, st = run_gpu(B, C0, 1.0, 0.01, 60, 20, options={"rhs3": 1})
     assert np.abs(C - Ct).max() <= 1e-13
     assert_series_close(s, st, 1e-12)
+    Cs, ss = run_gpu(B, C0, 1.0, 0.01, 60, 20, options={"sweep3": 1})      # separate x and y sweeps instead of the plane kernel
+    assert np.abs(C - Cs).max() <= 1e-13
+    assert_series_close(s, ss, 1e-12)
     sub = [0, 5, 11]
     Co, so = oracle.run(C0[sub], 1.0, 0.01, 60, 20)
     assert np.abs(C[sub] - Co).max() <= FIELD_TOL
     assert_series_close(s[:, sub], so)
+
+
+def test_3d_plane_sweep_paper_regime(B, oracle):
+    """x + y sweeps of a z-plane in one kernel at gamma dt = 529 (long closures: shuffle scan in x, K-term sum in y),
+    64^3 and 128^3, against the oracle."""
+    for N, M, nsteps in ((64, 2, 20), (128, 1, 6)):
+        C0 = inputs.initial_state(range(3300, 3300 + M), N, 3, -0.3, 0.1)
+        e = B.Ensemble(M, N, 3, 66.4, 7.97)
+        assert B.ch_get_option(e.ctx, "sweep_xy") == 1
+        e.close()
+        C, s = run_gpu(B, C0, 66.4, 7.97, nsteps, 2)
+        Co, so = oracle.run(C0, 66.4, 7.97, nsteps, 2)
+        assert np.abs(C - Co).max() <= 1e-9, N
+        assert_series_close(s, so, 1e-7)
 
 
 def test_small_3d_1000_steps(B, oracle):
