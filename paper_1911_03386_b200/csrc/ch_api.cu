@@ -304,6 +304,8 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         const int smem = N * N * 8 + 2 * (N / 16) * N * 8;
         cudaError_t e = N == 64 ? cudaFuncSetAttribute(k_sweep_xy_plane<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)
                                 : cudaFuncSetAttribute(k_sweep_xy_plane<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess && N == 128)
+            e = cudaFuncSetAttribute(k_sweep_xy_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 128 * 8 + 2 * 2 * 8 * 128 * 8);
         if (e != cudaSuccess) c->xy_ok = false;
         cudaGetLastError();
     }
@@ -514,7 +516,7 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         return CH_OK;
     }
     if (!strcmp(key, "sweep3")) {
-        if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: sweep3 must be 0 (auto) or 1 (separate x and y sweeps)");
+        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: sweep3 must be 0 (auto), 1 (separate x and y sweeps) or 2 (one CTA per plane)");
         ctx->opt_sweep3 = value;
         return CH_OK;
     }
@@ -716,8 +718,17 @@ static void launch_sweep_xy(ch_ctx *c, double *w)
     const int N = c->N;
     const size_t smem = (size_t)N * N * 8 + (size_t)2 * P * N * 8;
     const unsigned planes = (unsigned)((size_t)c->M * N);
-    if (N == 64) k_sweep_xy_plane<64><<<planes, 256, smem, c->stream>>>(prm, w);
-    else k_sweep_xy_plane<128><<<planes, 1024, smem, c->stream>>>(prm, w);
+    if (N == 64) { k_sweep_xy_plane<64><<<planes, 256, smem, c->stream>>>(prm, w); return; }
+    if (c->opt_sweep3 == 2) { k_sweep_xy_plane<128><<<planes, 1024, smem, c->stream>>>(prm, w); return; }
+    // N = 128: half a plane per CTA, clusters of 2 (two CTAs of different planes per SM overlap load and compute)
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.gridDim = dim3(2 * planes); cfg.blockDim = dim3(512);
+    cfg.dynamicSmemBytes = (size_t)64 * 128 * 8 + (size_t)2 * 2 * 8 * 128 * 8;
+    cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_sweep_xy_pair, prm, w);
 }
 
 // ---- fused 2D step: (RHS + y-sweep) then (x-sweep + update) ------------------------------------

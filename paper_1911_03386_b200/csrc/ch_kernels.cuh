@@ -581,3 +581,84 @@ __global__ void __launch_bounds__(NC * NC / 16, NC == 64 ? 3 : 1) k_sweep_xy_pla
         for (int k = 0; k < LC; ++k) o[k * NC] = v[k];
     }
 }
+
+// ------------------------------------------------------------------------------------
+// k_sweep_xy_pair: the plane kernel for N = 128 on a thread-block cluster of 2 CTAs, each holding half
+// the plane (64 rows x 128 columns, 64 KB), so that two CTAs of different planes share an SM and one
+// loads while the other computes.  x phase as in k_sweep_xy_plane (rows are complete in a CTA).
+// y phase: thread (column, local chunk of 16 rows); every chunk state is written to the local exchange
+// arrays AND to the peer CTA's (distributed shared memory), one cluster barrier per direction, then the
+// usual K-term closure over all 8 chunks.  grid = 2 * planes, cluster (2,1,1), block 512,
+// dynamic smem = 64 KB + 2 directions * 2 * 8 * 128 * 8 B.
+// ------------------------------------------------------------------------------------
+__device__ __forceinline__ void pair_store_remote(double *local, unsigned peer, double v)
+{
+    unsigned ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(ra) : "r"((unsigned)__cvta_generic_to_shared(local)), "r"(peer));
+    asm volatile("st.shared::cluster.f64 [%0], %1;\n" ::"r"(ra), "d"(v) : "memory");
+}
+__device__ __forceinline__ void pair_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+
+__global__ void __launch_bounds__(512, 2) k_sweep_xy_pair(const __grid_constant__ SweepParams prm, double *__restrict__ w)
+{
+    constexpr int NC = 128, LC = 16, P = NC / LC, HR = NC / 2, NT = 512, G = HR * NC / 2;     // G granules per half plane
+    extern __shared__ double2 sl[];
+    double *sxf = reinterpret_cast<double *>(sl + G), *sxb = sxf + 2 * P * NC;                // [a|b][chunk][column] per direction
+    const int t = threadIdx.x;
+    unsigned rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(rank));
+    const unsigned peer = rank ^ 1u;
+    const size_t plane = blockIdx.x >> 1;
+    double *wp = w + plane * NC * NC + (size_t)rank * HR * NC;
+    double2 *g2 = reinterpret_cast<double2 *>(wp);
+#pragma unroll
+    for (int k = 0; k < G / NT; ++k) ck_cp_async16(&sl[swz<LC>(k * NT + t)], g2 + k * NT + t);
+    ck_cp_async_wait_all();
+    __syncthreads();
+    double v[LC];
+    {   // x phase: rows of this half
+        const int l = t / P, c = t - l * P, gbase = l * (NC / 2) + c * (LC / 2);
+#pragma unroll
+        for (int k = 0; k < LC / 2; ++k) { const double2 x = sl[swz<LC>(gbase + k)]; v[2 * k] = x.x; v[2 * k + 1] = x.y; }
+        chunk_solve_scan<LC>(prm, v, c, nullptr);
+#pragma unroll
+        for (int k = 0; k < LC / 2; ++k) sl[swz<LC>(gbase + k)] = make_double2(v[2 * k], v[2 * k + 1]);
+    }
+    __syncthreads();
+    {   // y phase: column x, local chunk cl (global chunk c = rank * 4 + cl)
+        const int x = t % NC, cl = t / NC, c = (int)rank * (P / 2) + cl;
+        const double *sd = reinterpret_cast<const double *>(sl);
+#pragma unroll
+        for (int k = 0; k < LC; ++k) {
+            const int g = (cl * LC + k) * (NC / 2) + (x >> 1);
+            v[k] = sd[2 * swz<LC>(g) + (x & 1)];
+        }
+        const double np = prm.np, nq = prm.nq;
+        double a, b;
+        v[1] = fma(np, v[0], v[1]);
+#pragma unroll
+        for (int k = 2; k < LC; ++k) v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k]));
+        double *fa = sxf + c * NC + x, *fb = sxf + (P + c) * NC + x;
+        *fa = v[LC - 1]; *fb = v[LC - 2];
+        pair_store_remote(fa, peer, v[LC - 1]); pair_store_remote(fb, peer, v[LC - 2]);
+        pair_sync();
+        chunk_state_in<LC>(prm, sxf + x, sxf + P * NC + x, c, NC, +1, a, b);
+#pragma unroll
+        for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
+        v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
+#pragma unroll
+        for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
+        double *ba = sxb + c * NC + x, *bb = sxb + (P + c) * NC + x;
+        *ba = v[0]; *bb = v[1];
+        pair_store_remote(ba, peer, v[0]); pair_store_remote(bb, peer, v[1]);
+        pair_sync();
+        chunk_state_in<LC>(prm, sxb + x, sxb + P * NC + x, c, NC, -1, a, b);
+        double *o = wp + (size_t)cl * LC * NC + x;
+#pragma unroll
+        for (int k = 0; k < LC; ++k) o[k * NC] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
+    }
+    pair_sync();      // the peer may still be storing into this CTA's exchange arrays until both have passed the last read
+}

@@ -204,10 +204,11 @@ def test_3d_plane_sweep_paper_regime(B, oracle):
         e = B.Ensemble(M, N, 3, 66.4, 7.97)
         assert B.ch_get_option(e.ctx, "sweep_xy") == 1
         e.close()
-        C, s = run_gpu(B, C0, 66.4, 7.97, nsteps, 2)
         Co, so = oracle.run(C0, 66.4, 7.97, nsteps, 2)
-        assert np.abs(C - Co).max() <= 1e-9, N
-        assert_series_close(s, so, 1e-7)
+        for opts in (None, {"sweep3": 2}):               # N = 128: cluster pair / one CTA per plane
+            C, s = run_gpu(B, C0, 66.4, 7.97, nsteps, 2, options=opts)
+            assert np.abs(C - Co).max() <= 1e-9, (N, opts)
+            assert_series_close(s, so, 1e-7)
 
 
 def test_small_3d_1000_steps(B, oracle):
