@@ -282,3 +282,67 @@ def test_input_generator_is_order_independent_and_uniform():
     assert abs(u.mean()) < 0.01 and abs(u.var() - 1 / 3) < 0.01
     assert abs(np.corrcoef(u[:-1], u[1:])[0, 1]) < 0.01
     assert not np.array_equal(u[:10], inputs.uniform_pm1(43, 10))
+
+
+# ------------------------------------------------------------------ golden fixtures (tests/golden/*.txt)
+import os
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def golden_rows(name):
+    rows = []
+    for line in open(os.path.join(GOLDEN, name)):
+        if line.strip() and not line.startswith("#"):
+            rows.append(line.split())
+    return rows
+
+
+def test_golden_circulant_eigenvalues(oracle):
+    """Fourier modes are eigenvectors of the cyclic pentadiagonal matrix: the oracle's solve (banded and dense path)
+    must divide mode k by the stored lambda_k = 1 + sigma (2 - 2 cos(2 pi k/N))^2."""
+    rows = golden_rows("circulant_eigenvalues.txt")
+    assert len(rows) == 3 * 5 + 3 * 9
+    for N, sigma, k, lam in rows:
+        N, sigma, k, lam = int(N), float(sigma), int(k), float(lam)
+        i = np.arange(N)
+        b = np.stack([np.cos(2 * np.pi * k * i / N), np.sin(2 * np.pi * k * i / N) + (k == 0)])
+        for dense in (False, True):
+            v = oracle.solve_lines(b, sigma, dense=dense)
+            assert np.abs(v * lam - b).max() <= 1e-13 * lam, (N, sigma, k, dense)
+
+
+def test_golden_growth_factors(oracle):
+    """One oracle step of a small single Fourier mode against the stored closed-form growth factor."""
+    for D, N, mx, my, mz, cbar, gamma, dt, g in golden_rows("growth_factors.txt"):
+        D, N, ms = int(D), int(N), (int(mx), int(my), int(mz))[: int(D)]
+        cbar, gamma, dt, g = float(cbar), float(gamma), float(dt), float(g)
+        idx = np.meshgrid(*[np.arange(N)] * D, indexing="ij")            # [z][y][x]: last axis is x
+        phase = sum(2 * np.pi * m * ix / N for m, ix in zip(ms, idx[::-1]))
+        mode = np.cos(phase)
+        eps = 1e-7
+        C1 = oracle.step((cbar + eps * mode)[None], gamma, dt, 1)[0]
+        got = ((C1 - cbar) * mode).sum() / (eps * (mode * mode).sum())
+        assert abs(got - g) <= 2e-7 * max(1.0, abs(g)), (D, N, ms, cbar, got, g)
+
+
+def test_golden_kink_energy(oracle):
+    """Energy per unit length of the sampled tanh interface tends to the stored (2 sqrt 2 / 3) sqrt(gamma) as h -> 0."""
+    for gamma, sig in golden_rows("kink_energy.txt"):
+        gamma, sig = float(gamma), float(sig)
+        errs = []
+        for h, N in [(np.sqrt(gamma), 64), (np.sqrt(gamma) / 4, 256)]:
+            g = gamma / h ** 2                                          # h = 1 units: gamma' = gamma / h^2
+            e = oracle.energy(kink_pair(N, g), g)[0]
+            errs.append(abs(e[0] * h ** 2 / (2 * N * h) - sig) / sig)
+        assert errs[0] < 0.03 and errs[1] < 2e-3, (gamma, errs)
+
+
+def test_golden_table_a6_is_self_consistent():
+    """The paper's printed Table A.6: the order column equals log2 of the ratio of the printed E_n to within
+    their two printed digits, and tends to 1 (first order) -- the property the GPU study is compared with."""
+    rows = [(int(n), float(e), float(o)) for n, e, o in golden_rows("table_A6.txt")]
+    assert [r[0] for r in rows] == [128, 256, 512, 1024, 2048, 4096]
+    for (n, e, o), (_, e2, _) in zip(rows, rows[1:]):
+        assert abs(np.log2(e / e2) - o) < 0.06, n
+    assert abs(rows[-1][2] - 1.0) < 0.01 and abs(rows[-2][2] - 1.0) < 0.01
