@@ -245,7 +245,10 @@ __global__ void k_sweep_x_update(const __grid_constant__ SweepParams prm, const 
     extern __shared__ double2 sl[];
     const int P = prm.P;
     const int nthreads = blockDim.x, t = threadIdx.x;
-    const long long line0 = (long long)blockIdx.x * LPB;
+    // lines are taken from the END of the ensemble backwards: the fused RHS + y-sweep kernel before this one walks the
+    // members upwards, so its last ~100 MB of w and C are still in L2 -- and the C this kernel writes last (the first
+    // members) is what the next step's first tiles read
+    const long long line0 = (long long)(gridDim.x - 1 - blockIdx.x) * LPB;
     const int nlines = (int)((total_lines - line0) < LPB ? (total_lines - line0) : LPB);
     const int G = nlines * (N / 2);                           // 16-byte granules held by this CTA
     const double2 *gw = reinterpret_cast<const double2 *>(w + (size_t)line0 * N);
