@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 
 #include "ch_kernels.cuh"
+#include "ch_line2d.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -257,9 +258,10 @@ __global__ void k_sweep_x_update(const __grid_constant__ SweepParams prm, const 
     double *sa = reinterpret_cast<double *>(sC + (size_t)LPB * (N / 2));
     double *sb = sa + LPB * P;
 
-    for (int g = t; g < G; g += nthreads) cp_async16(&sl[swz<LC>(g)], gw + g);
+    const unsigned long long pol = l2_evict_first_policy();     // w is dead after this read; C is overwritten below
+    for (int g = t; g < G; g += nthreads) line_cp_async16_hint(&sl[swz<LC>(g)], gw + g, pol);
     cp_async_commit();
-    for (int g = t; g < G; g += nthreads) cp_async16(&sC[g], gC + g);
+    for (int g = t; g < G; g += nthreads) line_cp_async16_hint(&sC[g], gC + g, pol);
     cp_async_commit();
     cp_async_wait<1>();
     __syncthreads();

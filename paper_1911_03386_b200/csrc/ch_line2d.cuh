@@ -43,6 +43,19 @@ __device__ __forceinline__ void line_cp_async16(void *smem_dst, const void *gsrc
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gsrc) : "memory");
 }
+// same copy with an L2 evict-first hint: for streams that are read once (they should not displace what the NEXT
+// kernel will find in L2: the w this kernel writes, the C the previous kernel wrote)
+__device__ __forceinline__ unsigned long long l2_evict_first_policy()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void line_cp_async16_hint(void *smem_dst, const void *gsrc, unsigned long long policy)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gsrc), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void line_cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void line_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
