@@ -70,6 +70,7 @@ struct ch_ctx {
     int r3_parts, r3_resident;   // partials per member, CTAs resident on the device
     int opt_rhs3;                // 0 auto (streaming kernel when available), 1 tile kernel
     bool xy_ok;                  // 3D, N in {64, 128}: x- and y-sweep of a z-plane in one pass (k_sweep_xy_plane)
+    int dir3;                    // 3D: direction in which the next RHS launch walks the ensemble (alternates)
     int opt_sweep3;              // 0 auto (plane kernel when available), 1 separate x and y sweeps
     // fused 2D step, whole line in one CTA (ch_line2d.cuh)
     bool line_ok;
@@ -298,7 +299,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         }
         cudaGetLastError();
     }
-    c->opt_sweep3 = 0;
+    c->opt_sweep3 = 0; c->dir3 = 0;
     c->xy_ok = D == 3 && (N == 64 || N == 128) && c->chunked;
     if (c->xy_ok) {
         const int smem = N * N * 8 + 2 * (N / 16) * N * 8;
@@ -570,7 +571,7 @@ static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
     if (use_rhs3_stream(c)) {
         Rhs3Params p;
         p.gamma = c->gamma; p.mgam = -c->gamma; p.k1 = 6.0 * c->gamma - 1.0; p.scale = scale;
-        p.nunits = c->r3_parts * c->M; p.write = WRITE ? 1 : 0;
+        p.nunits = c->r3_parts * c->M; p.write = WRITE ? 1 : 0; p.rev = c->dir3;
         const int grid = p.nunits < c->r3_resident ? p.nunits : c->r3_resident;
         const size_t smem = rhs3_stream_smem(c->N);
         if (c->N == 64) k_rhs3d_stream<64, DIAG><<<grid, 256, smem, c->stream>>>(p, C, r, c->partials);
@@ -608,7 +609,7 @@ static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
     memcpy(p.beta, c->fac.beta, sizeof(p.beta));
     p.W = c->dW; p.K = c->fac.K; p.P = c->fac.P;
     // log-depth closure (contiguous-line kernels only): worth it once the K-term sum is long
-    p.scan = 0; p.scan2 = 0; p.S2 = c->dS2;
+    p.scan = 0; p.scan2 = 0; p.S2 = c->dS2; p.rev = 0;
     const int P = c->fac.P;
     if (c->opt_scan != 1 && (c->fac.K > 4 || c->opt_scan == 2) && P % 32 == 0 && P / 32 >= 2 && P / 32 <= 4) {
         p.scan2 = P / 32;
@@ -624,7 +625,7 @@ static void fill_params(const ch_ctx *c, SweepParams &p, double oscale)
 }
 
 // axis 0 = x, 1 = y, 2 = z.  update: C += result (last sweep of a step).  scale: multiply the output by oscale.
-static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale, double oscale)
+static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale, double oscale, int rev = 0)
 {
     const int N = c->N, D = c->D, M = c->M;
     const size_t n2 = (size_t)N * N, n3 = n2 * N;
@@ -663,6 +664,7 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
     }
     SweepParams prm;
     fill_params(c, prm, oscale);
+    prm.rev = rev;
     const int LC = c->LC, P = c->fac.P;
     if (axis == 0) {
         const long long total_lines = (long long)M * (D == 3 ? n2 : (size_t)N);
@@ -705,13 +707,13 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
 static bool use_fused(const ch_ctx *c) { return fuse_mode(c) != 0; }
 
 // 3D: x- and y-sweep of every z-plane in one pass
-static void launch_sweep_xy(ch_ctx *c, double *w)
+static void launch_sweep_xy(ch_ctx *c, double *w, int rev)
 {
     ProfScope ps(c, KIND_SWEEP_XY);
     SweepParams prm;
     fill_params(c, prm, 1.0);
     const int P = c->fac.P;
-    prm.scan = 0; prm.scan2 = 0;
+    prm.scan = 0; prm.scan2 = 0; prm.rev = rev;
     while ((1 << prm.scan) < P) ++prm.scan;
     memcpy(prm.Mp, c->fac.Mpow2, sizeof(prm.Mp));
     memcpy(prm.Wc, c->fac.Wclose, sizeof(prm.Wc));
@@ -914,8 +916,11 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
         }
         if (fused) launch_sweep_x_update(ctx, unscaled);
         else if (D == 3 && ctx->xy_ok && ctx->opt_sweep3 != 1 && ctx->opt_sweep != 1) {
-            launch_sweep_xy(ctx, ctx->w);
-            launch_sweep(ctx, ctx->w, 2, true, false, 1.0);
+            // RHS walks the ensemble in direction dir3, the plane kernel back, the z-sweep forth again, and the next
+            // step starts from where this one ended: each kernel finds the tail of its predecessor's output in L2
+            launch_sweep_xy(ctx, ctx->w, !ctx->dir3);
+            launch_sweep(ctx, ctx->w, 2, true, false, 1.0, ctx->dir3);
+            ctx->dir3 = !ctx->dir3;
         }
         else for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
         ctx->n++;

@@ -24,6 +24,7 @@ struct SweepParams {
     double Mp[5][4];            // M^(2^k)
     double Wc[4];               // (I - M^P)^-1
     int scan;                   // 0, or log2 P (P a power of two, 2 <= P <= 32)
+    int rev;                    // 3D sweeps: walk the blocks from the last to the first (L2 reuse between consecutive kernels)
     int scan2;                  // 0, or W = P / 32 in 2..4: two-level scan (warp scan + W warp aggregates)
     const double *S2;           // device: Mlane[32][4] then WG[4][4] (ch_factor.h)
 };
@@ -378,7 +379,8 @@ __global__ void __launch_bounds__(512) k_sweep_strided(const __grid_constant__ S
     extern __shared__ double sx[];
     const int COLS = blockDim.x, P = blockDim.y;
     const int tx = threadIdx.x, c = threadIdx.y;
-    const int ib = blockIdx.x % inner_blocks, o = blockIdx.x / inner_blocks;
+    const unsigned bid = prm.rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int ib = bid % inner_blocks, o = bid / inner_blocks;
     const size_t base = (size_t)o * outer_stride + (size_t)c * LC * line_stride + (size_t)ib * COLS + tx;
     double *sa = sx + tx, *sb = sx + P * COLS + tx;
 
@@ -552,7 +554,8 @@ __global__ void __launch_bounds__(NC * NC / 16, NC == 64 ? 3 : 1) k_sweep_xy_pla
     extern __shared__ double2 sl[];
     double *sx = reinterpret_cast<double *>(sl + G);
     const int t = threadIdx.x;
-    double2 *g2 = reinterpret_cast<double2 *>(w + (size_t)blockIdx.x * NC * NC);
+    const unsigned bid = prm.rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    double2 *g2 = reinterpret_cast<double2 *>(w + (size_t)bid * NC * NC);
 #pragma unroll
     for (int k = 0; k < G / NT; ++k) ck_cp_async16(&sl[swz<LC>(k * NT + t)], g2 + k * NT + t);
     ck_cp_async_wait_all();
@@ -576,7 +579,7 @@ __global__ void __launch_bounds__(NC * NC / 16, NC == 64 ? 3 : 1) k_sweep_xy_pla
             v[k] = sd[2 * swz<LC>(g) + (x & 1)];
         }
         chunk_solve<LC>(prm, v, sx + x, sx + P * NC + x, c, NC);      // the strided closure sums K terms through shared memory
-        double *o = w + (size_t)blockIdx.x * NC * NC + (size_t)c * LC * NC + x;
+        double *o = w + (size_t)bid * NC * NC + (size_t)c * LC * NC + x;
 #pragma unroll
         for (int k = 0; k < LC; ++k) o[k * NC] = v[k];
     }
@@ -611,7 +614,7 @@ __global__ void __launch_bounds__(512, 2) k_sweep_xy_pair(const __grid_constant_
     unsigned rank;
     asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(rank));
     const unsigned peer = rank ^ 1u;
-    const size_t plane = blockIdx.x >> 1;
+    const size_t plane = prm.rev ? (gridDim.x >> 1) - 1 - (blockIdx.x >> 1) : (blockIdx.x >> 1);
     double *wp = w + plane * NC * NC + (size_t)rank * HR * NC;
     double2 *g2 = reinterpret_cast<double2 *>(wp);
 #pragma unroll

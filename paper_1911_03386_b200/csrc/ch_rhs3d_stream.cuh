@@ -29,7 +29,7 @@
 
 struct Rhs3Params {
     double gamma, mgam, k1, scale;      // mu = c (c^2 + k1) - gamma * (sum of the 6 neighbours), k1 = 6 gamma - 1
-    int nunits, write;
+    int nunits, write, rev;             // rev: take the units from the last to the first
 };
 
 static inline size_t rhs3_stream_smem(int N)
@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(4 * NC, 1) k_rhs3d_stream(const __grid_constan
     double2 *exC = sm2 + (size_t)3 * RY * NT, *exM = exC + 2 * 2 * NHW * 16;
     const double mgam = prm.mgam, k1 = prm.k1, scale = prm.scale;
 
-    for (int unit = blockIdx.x; unit < prm.nunits; unit += gridDim.x) {
+    for (int u = blockIdx.x; u < prm.nunits; u += gridDim.x) {
+        const int unit = prm.rev ? prm.nunits - 1 - u : u;
         const int zr = unit % NZ, t = unit / NZ, strip = t % strips, m = t / strips;
         const int X = strip * R3_VALID, z0 = zr * ZR;
         int gx = X - 2 + 2 * li;
