@@ -121,14 +121,22 @@ long long ch_step_count(const ch_ctx *ctx);
 int ch_rhs(ch_ctx *ctx, double *r_out, int on_device);
 int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
 
-/* Kernel-variant options (measurement knobs; every variant computes the same step):
- *   "sweep"   0 auto, 1 force the generic thread-per-line sweeps, 2 force the chunked sweeps
- *   "fuse"    0 auto (D = 2, N % 16 == 0: the fused step -- RHS fused into the y-sweep, then the x-sweep
- *             fused with C += w; 40 instead of 56 bytes per grid-point update), 1 force the three-pass
- *             step (RHS, x-sweep, y-sweep + update), 2 require the fused step
- * ch_get_option also answers "chunked" (chunk length of the fast sweeps, 0 if N needs the
- * generic path), "K" (chunk neighbours summed by the periodic closure) and "fused" (thread-block
- * cluster size of the fused 2D step, 0 if this shape has none). */
+/* Kernel-variant options (measurement knobs; every variant computes the same step to round-off):
+ *   "sweep"    0 auto, 1 force the generic thread-per-line sweeps, 2 force the chunked periodic-LU sweeps,
+ *              3 parallel cyclic reduction for the x-axis of ch_sweep (N a power of two <= 4096)
+ *   "fuse"     which 2D step runs: 0 auto, 1 three passes (RHS, x-sweep, y-sweep + update; 56 B per update),
+ *              2 RHS fused into a cluster/st.async y-sweep, 3 the line kernel (N in {32, 64, 96, 128, 192, 256,
+ *              384, 512}), 4 the cluster line kernel (N in {1024, 2048, 4096}); modes 2-4 finish with the
+ *              x-sweep fused with C += w (40 B per update).  A mode the shape does not support is CH_EINVAL.
+ *   "linesync" line kernel: 0 auto (neighbour-warp flags when the closure is truncated to 2 chunks), 1 CTA barriers
+ *   "scan"     closure of the chunk states: 0 auto (log-depth shuffle scan when the K-term sum is long), 1 K-term
+ *              sum always, 2 scan wherever it is available
+ *   "rhs3"     3D RHS: 0 auto (z-marching kernel for N in {64, 128}), 1 tile kernel
+ *   "sweep3"   3D x/y sweeps: 0 auto (one pass per z-plane in shared memory for N in {64, 128}; cluster pairs at
+ *              N = 128), 1 separate x- and y-sweeps, 2 one CTA per plane
+ * ch_get_option answers these and, read-only: "chunked" (chunk length of the fast sweeps, 0 if N needs the generic
+ * path), "K" (chunks summed by the periodic closure), "fused" / "line" / "cline" / "rhs3_stream" / "sweep_xy"
+ * (non-zero if this shape has that kernel), "fuse_mode" (the 2D step that will run: 0, 2, 3 or 4). */
 int ch_set_option(ch_ctx *ctx, const char *key, int value);
 int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
 
