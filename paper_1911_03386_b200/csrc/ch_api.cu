@@ -549,6 +549,10 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "chunked")) { *value = ctx->chunked ? ctx->LC : 0; return CH_OK; }
     if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
     if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
+    if (!strcmp(key, "linesync")) { *value = ctx->opt_linesync; return CH_OK; }
+    if (!strcmp(key, "scan")) { *value = ctx->opt_scan; return CH_OK; }
+    if (!strcmp(key, "rhs3")) { *value = ctx->opt_rhs3; return CH_OK; }
+    if (!strcmp(key, "sweep3")) { *value = ctx->opt_sweep3; return CH_OK; }
     if (!strcmp(key, "fused")) { *value = ctx->fused_ok ? ctx->f_CS : 0; return CH_OK; }
     if (!strcmp(key, "sweep_xy")) { *value = (ctx->xy_ok && ctx->opt_sweep3 != 1 && ctx->opt_sweep != 1) ? 1 : 0; return CH_OK; }
     if (!strcmp(key, "rhs3_stream")) { *value = use_rhs3_stream(ctx) ? ctx->r3_resident : 0; return CH_OK; }
