@@ -290,6 +290,8 @@ def run_ours(args):
             cpu = {"value": None, "unit": UNIT, "cores": 0, "kind": "oracle", "sample": "skipped (--no-cpu-baseline)"}
         else:
             cpu = oracle_sample(name, max(5, int(1.5e8 / N ** D)))    # ~10-20 s of CPU work per core
+            one = oracle_sample(name, max(2, int(3e7 / N ** D)), max_members=1)   # one member on one thread, a few seconds
+            cpu["value_1thread"] = one["value"]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": secs / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -299,7 +301,7 @@ def run_ours(args):
                        "sampling": f"F, dF/dt, beta, mass every {stride} steps inside the timed region"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "roofline": roofline, "kernels": kernels, "paper_regime": paper_regime,
-            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "value_1thread") if k in cpu},
         }
         print(json.dumps(line))
     if world > 1:
