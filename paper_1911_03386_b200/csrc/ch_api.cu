@@ -55,6 +55,13 @@ struct ch_ctx {
     cudaStream_t stream;
     // options
     int opt_sweep;          // 0 auto, 1 generic, 2 chunked
+    // CUDA graph of CH_GRAPH_STEPS plain (non-sampling) steps for launch-bound (small) ensembles
+    int opt_graph;          // 0 auto (graphs when the ensemble has <= 8 Mi points), 1 off, 2 always
+    cudaGraphExec_t gexec;
+    cudaStream_t cap_stream;
+    long long gsig;         // option signature the graph was captured with
+    long long glaunches;    // kernel nodes in the graph
+    bool graph_broken;      // capture failed once: plain launches from then on
     int opt_scan;           // contiguous sweeps: 0 auto (shuffle-scan closure when K > 4), 1 off, 2 always
     int opt_linesync;       // line kernel: 0 auto (neighbour-warp sync when K <= 2), 1 CTA barriers
     int opt_fuse;           // 0 auto (fused 2D step when available), 1 off, 2 cluster kernel, 3 line kernel
@@ -249,7 +256,8 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->C = c->w = c->partials = c->eout = nullptr;
     c->has_state = false; c->n = 0; c->t0 = 0.0;
     c->series = nullptr; c->stride = 0; c->capacity = 0; c->cursor = 0; c->last_sampled = -1;
-    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->opt_scan = 0; c->launches = 0; c->profiling = false;
+    c->stream = 0; c->opt_sweep = 0; c->opt_fuse = 0; c->opt_linesync = 0; c->opt_scan = 0;
+    c->opt_graph = 0; c->gexec = nullptr; c->cap_stream = nullptr; c->gsig = -1; c->glaunches = 0; c->graph_broken = false; c->launches = 0; c->profiling = false;
     c->f_CPB = c->f_CS = c->f_strips = 0;
     c->fused_ok = fused_geometry(N, D, &c->f_CPB, &c->f_CS, &c->f_strips);
     c->cline_ok = false; c->cl_CS = 0; c->cl_strips = 0; c->cl_resident = 0;
@@ -403,6 +411,8 @@ extern "C" int ch_destroy(ch_ctx *ctx)
     if (ctx->dW16) cudaFree(ctx->dW16);
     if (ctx->dS2) cudaFree(ctx->dS2);
     if (ctx->dS2c) cudaFree(ctx->dS2c);
+    if (ctx->gexec) cudaGraphExecDestroy(ctx->gexec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     if (ctx->dS2_16) cudaFree(ctx->dS2_16);
     delete ctx;
     return CH_OK;
@@ -511,6 +521,11 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_sweep = value;
         return CH_OK;
     }
+    if (!strcmp(key, "graph")) {
+        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: graph must be 0 (auto), 1 (off) or 2 (always)");
+        ctx->opt_graph = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "scan")) {
         if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: scan must be 0 (auto), 1 (off) or 2 (always)");
         ctx->opt_scan = value;
@@ -550,6 +565,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "K")) { *value = ctx->fac.K; return CH_OK; }
     if (!strcmp(key, "fuse")) { *value = ctx->opt_fuse; return CH_OK; }
     if (!strcmp(key, "linesync")) { *value = ctx->opt_linesync; return CH_OK; }
+    if (!strcmp(key, "graph")) { *value = ctx->opt_graph; return CH_OK; }
     if (!strcmp(key, "scan")) { *value = ctx->opt_scan; return CH_OK; }
     if (!strcmp(key, "rhs3")) { *value = ctx->opt_rhs3; return CH_OK; }
     if (!strcmp(key, "sweep3")) { *value = ctx->opt_sweep3; return CH_OK; }
@@ -893,6 +909,67 @@ static int check_launch(ch_ctx *ctx, const char *what)
     return CH_OK;
 }
 
+// one time step; sample: also reduce F, Fdot, mass of C^n and write the series entry
+static void launch_one_step(ch_ctx *ctx, bool sample)
+{
+    const int D = ctx->D;
+    const bool fused = use_fused(ctx);
+    bool unscaled = false;
+    if (fused) unscaled = launch_rhs_sweep_y(ctx, sample, true);
+    else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
+    if (sample) {
+        launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
+                      fused ? fused_parts(ctx) : rhs_parts_in_use(ctx));
+        ctx->cursor++; ctx->last_sampled = ctx->n;
+    }
+    if (fused) launch_sweep_x_update(ctx, unscaled);
+    else if (D == 3 && ctx->xy_ok && ctx->opt_sweep3 != 1 && ctx->opt_sweep != 1) {
+        // RHS walks the ensemble in direction dir3, the plane kernel back, the z-sweep forth again, and the next
+        // step starts from where this one ended: each kernel finds the tail of its predecessor's output in L2
+        launch_sweep_xy(ctx, ctx->w, !ctx->dir3);
+        launch_sweep(ctx, ctx->w, 2, true, false, 1.0, ctx->dir3);
+        ctx->dir3 = !ctx->dir3;
+    }
+    else for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
+}
+
+// CUDA graph of CH_GRAPH_STEPS plain steps (their launches do not depend on the step index).  Captured on an
+// internal stream (the caller's may be the legacy default stream, which cannot be captured) and replayed on
+// the caller's.  Small ensembles are launch bound: CFG1's two 4096-point kernels per step.
+#define CH_GRAPH_STEPS 8
+static bool graph_wanted(const ch_ctx *c)
+{
+    if (c->opt_graph == 1 || c->graph_broken || c->profiling) return false;
+    return c->opt_graph == 2 || c->total <= ((size_t)8 << 20);
+}
+
+static bool ensure_graph(ch_ctx *c)
+{
+    const long long sig = ((((((long long)c->opt_sweep * 8 + c->opt_fuse) * 4 + c->opt_linesync) * 4 + c->opt_scan) * 4 + c->opt_rhs3) * 4
+                           + c->opt_sweep3);
+    if (c->gexec && c->gsig == sig) return true;
+    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); c->graph_broken = true; return false;
+    }
+    cudaStream_t user = c->stream;
+    const long long l0 = c->launches;
+    const int dir0 = c->dir3;
+    cudaGraph_t g = nullptr;
+    c->stream = c->cap_stream;
+    cudaError_t e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        for (int i = 0; i < CH_GRAPH_STEPS; ++i) launch_one_step(c, false);
+        e = cudaStreamEndCapture(c->cap_stream, &g);
+    }
+    c->stream = user; c->glaunches = c->launches - l0; c->launches = l0; c->dir3 = dir0;
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec, g, 0);
+    if (g) cudaGraphDestroy(g);
+    if (e != cudaSuccess) { cudaGetLastError(); c->gexec = nullptr; c->graph_broken = true; return false; }
+    c->gsig = sig;
+    return true;
+}
+
 extern "C" int ch_step(ch_ctx *ctx, int nsteps)
 {
     if (!ctx) return CH_EINVAL;
@@ -906,28 +983,27 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
         if (first == ctx->last_sampled) cnt -= 1;
         if (ctx->cursor + cnt > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_step: series full");
     }
-    const int D = ctx->D;
-    const bool fused = use_fused(ctx);
-    for (int s = 0; s < nsteps; ++s) {
+    const bool graphs = graph_wanted(ctx);
+    for (int s = 0; s < nsteps;) {
         const bool sample = ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n;
-        bool unscaled = false;
-        if (fused) unscaled = launch_rhs_sweep_y(ctx, sample, true);
-        else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
-        if (sample) {
-            launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
-                          fused ? fused_parts(ctx) : rhs_parts_in_use(ctx));
-            ctx->cursor++; ctx->last_sampled = ctx->n;
+        if (!sample && graphs && ctx->dir3 == 0) {
+            // plain steps ahead of the next sampling step (or of the end of this call)
+            long long plain = nsteps - s;
+            if (ctx->series) {
+                const long long r = ctx->n % ctx->stride, until = r == 0 ? ctx->stride : ctx->stride - r;
+                if (until < plain) plain = until;
+            }
+            if (plain >= CH_GRAPH_STEPS && ensure_graph(ctx)) {
+                if (cudaGraphLaunch(ctx->gexec, ctx->stream) == cudaSuccess) {
+                    ctx->launches += ctx->glaunches;
+                    ctx->n += CH_GRAPH_STEPS; s += CH_GRAPH_STEPS;
+                    continue;
+                }
+                cudaGetLastError(); ctx->graph_broken = true;
+            }
         }
-        if (fused) launch_sweep_x_update(ctx, unscaled);
-        else if (D == 3 && ctx->xy_ok && ctx->opt_sweep3 != 1 && ctx->opt_sweep != 1) {
-            // RHS walks the ensemble in direction dir3, the plane kernel back, the z-sweep forth again, and the next
-            // step starts from where this one ended: each kernel finds the tail of its predecessor's output in L2
-            launch_sweep_xy(ctx, ctx->w, !ctx->dir3);
-            launch_sweep(ctx, ctx->w, 2, true, false, 1.0, ctx->dir3);
-            ctx->dir3 = !ctx->dir3;
-        }
-        else for (int axis = 0; axis < D; ++axis) launch_sweep(ctx, ctx->w, axis, axis == D - 1, false, 1.0);
-        ctx->n++;
+        launch_one_step(ctx, sample);
+        ctx->n++; ++s;
     }
     if (ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n) {
         const int np_ = launch_diag_only(ctx);

@@ -387,6 +387,24 @@ def test_steady_state_and_split_calls(B, oracle):
     e.close()
 
 
+@pytest.mark.parametrize("M,N,D", [(1, 64, 2), (3, 256, 2), (2, 32, 3), (1, 64, 3), (2, 24, 2)])
+def test_cuda_graph_replay_is_bitwise_the_plain_launches(B, M, N, D):
+    """Small ensembles are launch bound: ch_step replays a CUDA graph of 8 plain steps between sampling steps.
+    Same field, same series, same launch count as plain launches, also across split calls and odd step counts."""
+    C0 = inputs.initial_state(range(90, 90 + M), N, D, -0.2, 0.1)
+    out = {}
+    for g in (1, 2):
+        e = B.Ensemble(M, N, D, 1.0, 0.01, options={"graph": g})
+        e.set_state(C0)
+        e.set_series(40, 6)
+        for k in (37, 1, 90, 16, 33):                    # 177 steps: graphs start at every phase of the stride
+            e.step(k)
+        out[g] = (e.get_state(), e.series(), B.ch_launch_count(e.ctx))
+        e.close()
+    assert np.array_equal(out[1][0], out[2][0]) and np.array_equal(out[1][1], out[2][1])
+    assert out[1][2] == out[2][2] and out[1][1].shape[0] == 5
+
+
 def test_errors_and_edge_cases(B):
     e = B.Ensemble(1, 16, 2, 1.0, 0.01)
     with pytest.raises(B.ChError) as ei:
