@@ -11,9 +11,11 @@
 // feeds r straight into the chunked periodic-LU recurrence of ch_factor.h, whose 2-double chunk states
 // are exchanged through shared memory (the whole line is in this CTA: no cluster, no global traffic).
 // r and the forward/backward intermediates never exist in memory: 16 B per grid-point update.
-// A thread reads back only the rows it staged itself, so its staging slots are free as soon as its
-// forward pass is done: the loads of the CTA's NEXT tile are issued there and fly during the closure,
-// the backward pass and the write-out of the current tile.
+// A thread reads back only the rows it staged itself, so there is no barrier between load and compute and a
+// staging row is free a few rows after it was read: row k of the CTA's NEXT tile is issued from inside the
+// forward loop at row k, so the next tile's loads are in flight for a whole tile period without a second buffer.
+// Synchronisation of the chunk exchange: neighbour-warp release/acquire flags when the closure is truncated to
+// K <= 2 chunks (NB kernels), CTA barriers + K-term sum or log-depth shuffle scan otherwise.
 #pragma once
 
 #include <cuda_runtime.h>
