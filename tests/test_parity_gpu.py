@@ -242,6 +242,21 @@ def test_4096_lines_cluster_of_eight(B, oracle):
     assert_series_close(s, so)
 
 
+@pytest.mark.parametrize("name,nsteps", [("cfg4", 300), ("cfg5", 300), ("cfg2", 2000)])
+def test_full_size_invariants(B, name, nsteps):
+    """Properties that hold at any size, on the full configs in the launch configuration bench.py times:
+    mass conserved to round-off and F strictly decreasing for every member, beta finite."""
+    c = inputs.CONFIGS[name]
+    C0 = inputs.config_state(name)
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], nsteps, c["stride"])
+    mass, F = s[:, :, 3], s[:, :, 0]
+    scale = np.abs(C0).reshape(C0.shape[0], -1).sum(axis=1)
+    assert (np.abs(mass - mass[0]) <= 1e-12 * scale).all()
+    assert (np.diff(F, axis=0) < 0).all()
+    assert np.isfinite(s).all() and np.isfinite(C).all()
+    assert np.abs(C.reshape(C.shape[0], -1).sum(axis=1) - mass[-1]).max() <= 1e-9 * scale.max()
+
+
 def test_restart_parity_from_developed_state(B, oracle):
     """cbar = -0.4 is still linear at step 1000, so also compare from a coarsening state:
     GPU runs 10000 steps, the state is handed to both sides, compared after 1000 more."""
