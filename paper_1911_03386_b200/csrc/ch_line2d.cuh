@@ -34,6 +34,8 @@ struct LineParams {
     double W0[4], W1[4];            // first two closure matrices (all of them when K <= 2)
     const double *W;                // device [K][4] (ch_factor.h)
     int K, ntiles, write;
+    int M;                          // ensemble members in this launch
+    int nfull;                      // packed tiling (stepping kernels): tiles below nfull are full 28-column strips
     // log-depth closure of the barrier kernels when the K-term sum is long (ch_factor.h, Mpow2 / Wclose)
     double Mp[5][4], Wc[4];
     int scan;                       // 0, or log2 P (P a power of two)
@@ -147,6 +149,42 @@ __device__ __forceinline__ void line_scan_closure(const LineParams &prm, double2
     aA = sA.x; bA = sA.y; aB = sB.x; bB = sB.y;
 }
 
+// Tiling of the columns.  Plain: ceil(NC / 28) strips per member, the last one ragged.  Packed (stepping kernels,
+// when the NC % 28 leftover columns fit half a half-warp): the leftover strips of members 2j and 2j+1 share ONE
+// tile -- lanes 0..7 work on member 2j, lanes 8..15 on member 2j+1 -- so a ragged strip costs half a tile
+// (N = 512, 128 members: 2432 -> 2368 tiles = exactly 16 rounds of 148 CTAs).
+template <int NC>
+struct LineTiling {
+    static constexpr int SF = NC / LINE_VALID, REM = NC - SF * LINE_VALID;
+    static constexpr bool PACKABLE = REM > 0 && REM <= 12;
+};
+
+// member, first column (wrapped, even) and "produces output" of half-warp lane li in `tile`
+template <int NC, bool PACK>
+__device__ __forceinline__ void line_tile_decode(int tile, int nfull, int M, int li, int &m, int &gx, bool &ok)
+{
+    constexpr int strips = (NC + LINE_VALID - 1) / LINE_VALID, SF = LineTiling<NC>::SF, REM = LineTiling<NC>::REM;
+    if (!PACK) {
+        const int strip = tile % strips;
+        m = tile / strips;
+        gx = strip * LINE_VALID - 2 + 2 * li;
+        ok = li >= 1 && li < 15 && gx < NC;
+    } else if (tile < nfull) {
+        const int strip = tile % SF;
+        m = tile / SF;
+        gx = strip * LINE_VALID - 2 + 2 * li;
+        ok = li >= 1 && li < 15;
+    } else {
+        const int l8 = li & 7;
+        m = 2 * (tile - nfull) + (li >> 3);
+        gx = SF * LINE_VALID - 2 + 2 * l8;
+        ok = l8 >= 1 && l8 <= REM / 2 && m < M;
+        if (m >= M) m = M - 1;                  // odd ensemble: the second half of the last packed tile idles on valid memory
+    }
+    if (gx < 0) gx += NC;
+    if (gx >= NC) gx -= NC;
+}
+
 // NC = N at compile time (row offsets become immediates).
 // grid = min(ntiles, resident CTAs), block = NC threads (= 16 threads per chunk, P = NC / 16 even),
 // dynamic smem = 20 * NC * 16 (staging) + 2 * 2 * P * 16 * 16 (forward, backward exchange slots).
@@ -180,11 +218,10 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
     double2 *slotF = sm2 + (size_t)NR * NT, *slotB = slotF + 2 * P * LINE_SS;
 
     // C rows y0-2 .. y0+LC+1 of this thread's column pair; only the two halo rows on either end wrap
+    constexpr bool PACK = !DIAG && LineTiling<NC>::PACKABLE;
     auto tile_base = [&](int tile) {
-        const int strip = tile % strips, m = tile / strips;
-        int gx = strip * LINE_VALID - 2 + 2 * li;
-        if (gx < 0) gx += N;
-        if (gx >= N) gx -= N;
+        int m, gx; bool ok;
+        line_tile_decode<NC, PACK>(tile, prm.nfull, prm.M, li, m, gx, ok);
         return C + (size_t)m * n2 + gx + (ptrdiff_t)(y0 - 2) * N;
     };
     auto load_row = [&](const double *p, int j) {     // j is a compile-time constant after unrolling
@@ -331,9 +368,9 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
             else line_state_in<P, SS>(prm, slotB, tid, -1, aA, bA, aB, bB);
             // where this thread's results go, recomputed from the tile and thread index
             const int t2 = opaque(tile), tid2 = opaque(tid);
-            const int strip2 = t2 % strips, m2 = t2 / strips, li2 = tid2 & 15;
-            const int gx = strip2 * LINE_VALID - 2 + 2 * li2;
-            if (li2 >= 1 && li2 < 15 && gx < N) {                   // producing lanes: 0 <= gx < N
+            int m2, gx; bool ok2;
+            line_tile_decode<NC, PACK>(t2, prm.nfull, prm.M, tid2 & 15, m2, gx, ok2);
+            if (ok2) {                                              // producing lanes: 0 <= gx < N
                 double2 *wm = reinterpret_cast<double2 *>(w + (size_t)m2 * n2 + (size_t)(tid2 >> 4) * (LC * N) + gx);
 #pragma unroll
                 for (int k = 0; k < LC; ++k) {
