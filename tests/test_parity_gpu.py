@@ -297,7 +297,7 @@ def test_generic_paths_end_to_end(B, oracle):
         assert_series_close(s, so)
 
 
-@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 176, 256, 352, 384, 512, 592, 1024])
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 128, 176, 192, 256, 352, 384, 512, 592, 1024])
 @pytest.mark.parametrize("gamma,dt", [(1.0, 0.01), (66.4, 7.97)])
 def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     """Every 2D step variant against the oracle: the line-fused step (RHS + y-sweep with whole lines
