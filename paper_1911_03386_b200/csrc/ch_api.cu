@@ -790,10 +790,10 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
         }
     }
     p.ntiles = c->l_strips * c->M; p.write = write ? 1 : 0;
-    p.M = c->M; p.nfull = 0;
+    p.M = c->M;
     {   // stepping kernels pack the ragged leftover strips of two members into one tile (ch_line2d.cuh, LineTiling)
         const int SF = c->N / LINE_VALID, REM = c->N - SF * LINE_VALID;
-        if (!diag && REM > 0 && REM <= 12) { p.nfull = c->M * SF; p.ntiles = p.nfull + (c->M + 1) / 2; }
+        if (!diag && REM > 0 && REM <= 12) p.ntiles = (c->M / 2) * (2 * SF + 1) + (c->M & 1) * (SF + 1);
     }
     const int grid = p.ntiles < c->l_resident ? p.ntiles : c->l_resident;
     const size_t smem = line_smem(c->N);

@@ -35,7 +35,6 @@ struct LineParams {
     const double *W;                // device [K][4] (ch_factor.h)
     int K, ntiles, write;
     int M;                          // ensemble members in this launch
-    int nfull;                      // packed tiling (stepping kernels): tiles below nfull are full 28-column strips
     // log-depth closure of the barrier kernels when the K-term sum is long (ch_factor.h, Mpow2 / Wclose)
     double Mp[5][4], Wc[4];
     int scan;                       // 0, or log2 P (P a power of two)
@@ -159,27 +158,35 @@ struct LineTiling {
     static constexpr bool PACKABLE = REM > 0 && REM <= 12;
 };
 
-// member, first column (wrapped, even) and "produces output" of half-warp lane li in `tile`
+// member, first column (wrapped, even) and "produces output" of half-warp lane li in `tile`.
+// Packed order: members come in pairs; pair p owns the PT = 2 SF + 1 consecutive tiles p PT .. (p + 1) PT - 1:
+// SF full strips of member 2p, SF of member 2p + 1, then the tile their leftover strips share (so a member's
+// tiles are complete PT tiles after its pair started: the one-kernel step of ch_step2d relies on it).  An odd
+// ensemble ends with a lone member: SF full strips and a half-idle leftover tile.
 template <int NC, bool PACK>
-__device__ __forceinline__ void line_tile_decode(int tile, int nfull, int M, int li, int &m, int &gx, bool &ok)
+__device__ __forceinline__ void line_tile_decode(int tile, int M, int li, int &m, int &gx, bool &ok)
 {
     constexpr int strips = (NC + LINE_VALID - 1) / LINE_VALID, SF = LineTiling<NC>::SF, REM = LineTiling<NC>::REM;
+    constexpr int PT = 2 * SF + 1;
     if (!PACK) {
         const int strip = tile % strips;
         m = tile / strips;
         gx = strip * LINE_VALID - 2 + 2 * li;
         ok = li >= 1 && li < 15 && gx < NC;
-    } else if (tile < nfull) {
-        const int strip = tile % SF;
-        m = tile / SF;
-        gx = strip * LINE_VALID - 2 + 2 * li;
-        ok = li >= 1 && li < 15;
     } else {
-        const int l8 = li & 7;
-        m = 2 * (tile - nfull) + (li >> 3);
-        gx = SF * LINE_VALID - 2 + 2 * l8;
-        ok = l8 >= 1 && l8 <= REM / 2 && m < M;
-        if (m >= M) m = M - 1;                  // odd ensemble: the second half of the last packed tile idles on valid memory
+        const int pair = tile / PT, k = tile - pair * PT;
+        const bool lone = 2 * pair + 1 >= M;                 // last member of an odd ensemble
+        if (k < SF || (!lone && k < 2 * SF)) {
+            m = 2 * pair + (k >= SF);
+            gx = (k >= SF ? k - SF : k) * LINE_VALID - 2 + 2 * li;
+            ok = li >= 1 && li < 15;
+        } else {
+            const int l8 = li & 7;
+            m = 2 * pair + (li >> 3);
+            gx = SF * LINE_VALID - 2 + 2 * l8;
+            ok = l8 >= 1 && l8 <= REM / 2 && m < M;
+            if (m >= M) m = M - 1;              // the idle half works on valid memory and stores nothing
+        }
     }
     if (gx < 0) gx += NC;
     if (gx >= NC) gx -= NC;
@@ -221,7 +228,7 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
     constexpr bool PACK = !DIAG && LineTiling<NC>::PACKABLE;
     auto tile_base = [&](int tile) {
         int m, gx; bool ok;
-        line_tile_decode<NC, PACK>(tile, prm.nfull, prm.M, li, m, gx, ok);
+        line_tile_decode<NC, PACK>(tile, prm.M, li, m, gx, ok);
         return C + (size_t)m * n2 + gx + (ptrdiff_t)(y0 - 2) * N;
     };
     auto load_row = [&](const double *p, int j) {     // j is a compile-time constant after unrolling
@@ -369,7 +376,7 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
             // where this thread's results go, recomputed from the tile and thread index
             const int t2 = opaque(tile), tid2 = opaque(tid);
             int m2, gx; bool ok2;
-            line_tile_decode<NC, PACK>(t2, prm.nfull, prm.M, tid2 & 15, m2, gx, ok2);
+            line_tile_decode<NC, PACK>(t2, prm.M, tid2 & 15, m2, gx, ok2);
             if (ok2) {                                              // producing lanes: 0 <= gx < N
                 double2 *wm = reinterpret_cast<double2 *>(w + (size_t)m2 * n2 + (size_t)(tid2 >> 4) * (LC * N) + gx);
 #pragma unroll
