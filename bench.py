@@ -40,7 +40,7 @@ NCU_TRAFFIC_BYTES = {
     # profiles/r01_v8_ncu_full_cfg3.md: one launch under `ncu --set full` (caches flushed before the launch, so the
     # L2 hits the live step gets from walking the ensemble up in one kernel and down in the next do not show; part of
     # the 268 MB write-back was still in L2 when the launch ended)
-    ("cfg3", "sweep_x_update"): 749.1e6,
+    ("cfg3", "sweep_x_update"): 749.5e6,
     ("cfg3", "rhs_sweep_y"): 487.9e6,
 }
 
