@@ -240,6 +240,9 @@ def run_ours(args):
                 "step_achieved_gbs": value / world * step_bytes / 1e9,
                 "step_frac": value / world * step_bytes / 1e9 / peak,
                 "step_frac_of_8TBs_nominal": value / world * step_bytes / 1e9 / 8000.0,
+                "note": ("achieved = algorithmic bytes / live CUDA-event time; a fraction above 1 means part of those bytes came from L2: "
+                         "consecutive kernels walk the ensemble in opposite directions, so each finds the tail of its predecessor's "
+                         "output in the 126 MB L2 (the ncu `traffic` figure is taken with caches flushed per launch)"),
                 "unfused_model_bytes_per_update": model_bytes,
                 "unfused_model_frac": value / world * model_bytes / 1e9 / peak}
 
