@@ -56,5 +56,24 @@ def kink():
     open(os.path.join(HERE, "kink_energy.txt"), "w").write("\n".join(out) + "\n")
 
 
+def dissipation():
+    out = ["# Leading-order dissipation of one Fourier mode C = cbar + eps cos(theta . i), theta_d = 2 pi m_d / N (eq. (4) P:34, eq. (6) P:64,",
+           "# readings G4/G5): mu = mubar + eps K cos(theta . i) + O(eps^2), K = (3 cbar^2 - 1) + gamma S, and with forward differences",
+           "# sum_i (mu_{i+e_d} - mu_i)^2 = eps^2 K^2 (N^D / 2) s_d, so  Fdot = - eps^2 K^2 (N^D / 2) sum_d s_d,  s_d = 2 - 2 cos theta_d, S = sum_d s_d.",
+           "# Each axis contributes its own s_d (all distinct below): a dropped, duplicated or swapped axis term changes the value.",
+           "# columns: D N m_x m_y m_z cbar gamma eps Fdot_leading per_axis_terms(x y z)"]
+    cases = [(3, 8, 1, 2, 3, "0", "1", "1e-5"), (3, 16, 2, 5, 7, "-0.4", "2", "1e-6"), (3, 12, 1, 4, 5, "0.3", "0.5", "1e-6"),
+             (2, 16, 3, 1, 0, "0", "1", "1e-5"), (2, 32, 5, 9, 0, "-0.4", "0.7", "1e-6")]
+    for D, N, mx, my, mz, cbar, gamma, eps in cases:
+        ms = (mx, my, mz)[:D]
+        s = [2 - 2 * mp.cos(2 * mp.pi * m / N) for m in ms]
+        S = sum(s)
+        cb, g_, e_ = mp.mpf(cbar), mp.mpf(gamma), mp.mpf(eps)
+        K = (3 * cb ** 2 - 1) + g_ * S
+        terms = [-e_ ** 2 * K ** 2 * mp.mpf(N) ** D / 2 * sd for sd in s] + [mp.mpf(0)] * (3 - D)
+        out.append(f"{D} {N} {mx} {my} {mz} {cbar} {gamma} {eps} {fmt(sum(terms))} " + " ".join(fmt(t) for t in terms))
+    open(os.path.join(HERE, "mode_dissipation.txt"), "w").write("\n".join(out) + "\n")
+
+
 if __name__ == "__main__":
-    eigenvalues(); growth(); kink()
+    eigenvalues(); growth(); kink(); dissipation()

@@ -191,6 +191,45 @@ def test_dissipation_matches_centred_difference_of_energy(oracle):
     assert np.median(rel) < 5e-3 and rel.max() < 5e-2
 
 
+@pytest.mark.parametrize("N,dt,seed", [(16, 0.0005, 5), (24, 0.0005, 6)])
+def test_dissipation_matches_centred_difference_of_energy_3d(oracle, N, dt, seed):
+    """The same pin in D = 3 (eq. (4), eq. (6)): every axis term of sum_d (mu_{i+e_d} - mu_i)^2 enters
+    (F^{n+1} - F^{n-1}) / (2 dt) ~ Fdot^n; dropping one axis is off by about a third."""
+    C0 = inputs.initial_state([seed], N, 3, 0.0, 0.1)
+    _, s = oracle.run(C0, 1.0, dt, 200, 1)
+    F, Fd = s[:, 0, 0], s[:, 0, 1]
+    fd = (F[2:] - F[:-2]) / (2 * dt)
+    rel = np.abs(fd - Fd[1:-1]) / np.abs(Fd[1:-1])
+    assert np.median(rel) < 5e-3 and rel.max() < 5e-2
+
+
+def _golden_rows(name):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    return [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+
+
+@pytest.mark.parametrize("row", _golden_rows("mode_dissipation.txt"), ids=lambda r: "D%sN%s_%s%s%s" % (r[0], r[1], r[2], r[3], r[4]))
+def test_single_mode_dissipation_closed_form(oracle, row):
+    """Closed form (tests/golden/mode_dissipation.txt, written by make_golden.py with mpmath): for
+    C = cbar + eps cos(theta . i), Fdot = -eps^2 K^2 (N^D / 2) sum_d s_d to leading order, each axis with its own s_d
+    (distinct), so a dropped / duplicated / swapped axis term in the oracle's dissipation sum fails (beta = -t Fdot / F, eq. (6)
+    P:64, is formed from this Fdot: test_run_series_convention)."""
+    D, N = int(row[0]), int(row[1])
+    m = [int(v) for v in row[2:5]][:D]
+    cbar, gamma, eps, Fd_exp = (float(v) for v in row[5:9])
+    idx = np.meshgrid(*[np.arange(N)] * D, indexing="ij")          # idx[0] is the slowest axis (z or y), idx[-1] is x
+    phase = sum(2 * np.pi * m[d] / N * idx[D - 1 - d] for d in range(D))     # m = (m_x, m_y, m_z)
+    C = (cbar + eps * np.cos(phase))[None]
+    Fd = oracle.energy(C, gamma)[0, 1]
+    # next order: mu has a 3 cbar eps^2 cos^2 term -> relative O(eps) corrections (O(eps^2) when cbar = 0)
+    assert abs(Fd - Fd_exp) <= (20 * eps * (abs(cbar) + eps) + 1e-9) * abs(Fd_exp)
+    # the oracle must tell the axes apart: permuting the mode numbers changes the closed form unless s_d are permuted too
+    if D == 3:
+        terms = [float(v) for v in row[9:12]]
+        assert len({round(t / Fd_exp, 6) for t in terms}) == 3
+
+
 def test_energy_of_random_initial_state_closed_form(oracle):
     """E[F(0)]/N^D = (cbar^4 + 2 cbar^2 A^2 + A^4/5 - 2 (cbar^2 + A^2/3) + 1)/4 + gamma D A^2/3
     for C0 = cbar + A U(-1,1) i.i.d. (pins both terms of F and the factor 1/2 gamma)."""
