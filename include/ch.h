@@ -127,7 +127,11 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *   "fuse"     which 2D step runs: 0 auto, 1 three passes (RHS, x-sweep, y-sweep + update; 56 B per update),
  *              2 RHS fused into a cluster/st.async y-sweep, 3 the line kernel (N in {32, 64, 96, 128, 192, 256,
  *              384, 512}), 4 the cluster line kernel (N in {1024, 2048, 4096}); modes 2-4 finish with the
- *              x-sweep fused with C += w (40 B per update).  A mode the shape does not support is CH_EINVAL.
+ *              x-sweep fused with C += w (40 B per update); 5 the one-pass local step:
+ *              RHS, y-sweep, x-sweep and update in one kernel that reads C^n once and writes C^{n+1} once (16 B per
+ *              update), legal when the recurrences of the factorisation decay within 18 points to below 2^-56 of the
+ *              data (gamma dt <~ 0.012; the bound is computed on the host, "local_reach"); auto picks it for D = 2,
+ *              N >= 256 when it is legal and the exact modes otherwise.  A mode the shape does not support is CH_EINVAL.
  *   "linesync" line kernel: 0 auto (neighbour-warp flags when the closure is truncated to 2 chunks), 1 CTA barriers
  *   "scan"     closure of the chunk states: 0 auto (log-depth shuffle scan when the K-term sum is long), 1 K-term
  *              sum always, 2 scan wherever it is available
@@ -138,14 +142,16 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *              N = 128), 1 separate x- and y-sweeps, 2 one CTA per plane
  * ch_get_option answers these and, read-only: "chunked" (chunk length of the fast sweeps, 0 if N needs the generic
  * path), "K" (chunks summed by the periodic closure), "fused" / "line" / "cline" / "rhs3_stream" / "sweep_xy"
- * (non-zero if this shape has that kernel), "fuse_mode" (the 2D step that will run: 0, 2, 3 or 4). */
+ * (non-zero if this shape has that kernel), "local" (non-zero if the one-pass local step is legal for this shape and
+ * gamma dt), "local_reach" (its decay reach H in points, -1 if above the limit), "fuse_mode" (the 2D step that will
+ * run: 0, 2, 3, 4 or 5). */
 int ch_set_option(ch_ctx *ctx, const char *key, int value);
 int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
 
 /* Per-kernel device timing.  ch_profile(ctx, 1) makes every later launch be bracketed by CUDA
  * events on the context's stream; ch_profile_read synchronises, returns the summed milliseconds
  * and launch counts per kernel kind (ch_kernel_kinds() kinds, named by ch_kernel_kind_name:
- * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z, rhs_sweep_y, rhs_sweep_y_diag, sweep_x_update, sweep_xy)
+ * rhs, rhs_diag, finish, sweep_x, sweep_y, sweep_z, rhs_sweep_y, rhs_sweep_y_diag, sweep_x_update, sweep_xy, step_local)
  * and clears the records. */
 int ch_profile(ch_ctx *ctx, int enable);
 int ch_profile_read(ch_ctx *ctx, double *ms, long long *counts, int nkinds);

@@ -18,10 +18,21 @@ from . import binding as B
 from . import inputs
 
 
+BASE_N, BASE_FACTOR = 64, 0.4     # time quantum tau = BASE_FACTOR * L / BASE_N; every run ends at the same multiple of tau
+
+
 def scaled_parameters(n, L, gamma, T, dt_factor):
+    """(gamma', dt', nsteps) in h = 1 units.  dt = dt_factor dx, so the step count must scale exactly with n and with
+    1 / dt_factor: the end time is fixed once as round(T / tau) tau, tau = BASE_FACTOR L / BASE_N, and
+    nsteps = round(T / tau) * (BASE_FACTOR / dt_factor) * (n / BASE_N).  (Rounding T / dt per grid would leave the coarse
+    and the fine field of eq. (A.1) one fine time step apart -- an O(dt) offset of the size of the error being measured.)"""
     dx = L / n
     dt = dt_factor * dx
-    nsteps = int(round(T / dt))
+    mult = (BASE_FACTOR / dt_factor) * (n / BASE_N)
+    if abs(mult - round(mult)) < 1e-9 and mult >= 1:
+        nsteps = int(round(T / (BASE_FACTOR * L / BASE_N))) * int(round(mult))
+    else:
+        nsteps = int(round(T / dt))
     return gamma / dx ** 2, dt / dx ** 2, nsteps
 
 

@@ -14,11 +14,12 @@
 #include "ch_line2d.cuh"
 #include "ch_rhs3d_stream.cuh"
 #include "ch_cline2d.cuh"
+#include "ch_local2d.cuh"
 
 enum { KIND_RHS = 0, KIND_RHS_DIAG, KIND_FINISH, KIND_SWEEP_X, KIND_SWEEP_Y, KIND_SWEEP_Z,
-       KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_SWEEP_XY, KIND_COUNT };
+       KIND_RHS_SWEEP_Y, KIND_RHS_SWEEP_Y_DIAG, KIND_SWEEP_X_UPDATE, KIND_SWEEP_XY, KIND_STEP_LOCAL, KIND_COUNT };
 static const char *const kKindNames[KIND_COUNT] = { "rhs", "rhs_diag", "finish", "sweep_x", "sweep_y", "sweep_z",
-                                                    "rhs_sweep_y", "rhs_sweep_y_diag", "sweep_x_update", "sweep_xy" };
+                                                    "rhs_sweep_y", "rhs_sweep_y_diag", "sweep_x_update", "sweep_xy", "step_local" };
 
 struct ProfRec { int kind; cudaEvent_t e0, e1; };
 
@@ -82,6 +83,9 @@ struct ch_ctx {
     // fused 2D step, whole line in one CTA (ch_line2d.cuh)
     bool line_ok;
     int l_strips, l_resident;    // column strips per member, CTAs resident on the device
+    // one-pass local 2D step for small gamma dt (ch_local2d.cuh)
+    bool local_ok;
+    int loc_H, loc_resident;     // decay reach (ch_factor_reach), CTAs resident on the device
     long long launches;
     bool profiling;
     std::vector<ProfRec> prof;
@@ -89,10 +93,14 @@ struct ch_ctx {
 };
 
 // which fused 2D step runs: 0 none (three-pass), 2 st.async cluster kernel, 3 line kernel, 4 cluster line kernel
-// (mode 4 steps with the cluster line kernel and samples with the mode-2 kernel)
+// (mode 4 steps with the cluster line kernel and samples with the tile RHS kernel), 5 one-pass local step (small
+// gamma dt only; samples with the line kernel's or the tile kernel's diagnostics-only launch)
+#define CH_LOCAL_AUTO_MIN_N 256
 static int fuse_mode(const ch_ctx *c)
 {
     if (c->opt_fuse == 1 || c->opt_sweep == 1) return 0;
+    if (c->opt_fuse == 5) return c->local_ok ? 5 : 0;
+    if (c->opt_fuse == 0 && c->local_ok && c->N >= CH_LOCAL_AUTO_MIN_N) return 5;
     if (c->opt_fuse == 2) return c->fused_ok ? 2 : 0;
     if (c->opt_fuse == 3) return c->line_ok ? 3 : 0;
     if (c->opt_fuse == 4) return c->cline_ok ? 4 : 0;
@@ -340,6 +348,21 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     }
     c->l_strips = 0; c->l_resident = 0;
     c->line_ok = line_geometry(N, D, &c->l_strips);
+    // one-pass local step: needs the decay reach of the recurrences within LOC_HMAX (gamma dt <~ 0.012)
+    c->local_ok = false; c->loc_H = -1; c->loc_resident = 0;
+    if (D == 2 && N % 4 == 0 && N >= 16) {
+        c->loc_H = ch_factor_reach(&c->fac, ldexp(1.0, -56), LOC_HMAX);
+        if (c->loc_H >= 0) {
+            if (c->loc_H < 2) c->loc_H = 2;
+            int per_sm = 0, dev = 0, sms = 0;
+            cudaError_t e = cudaFuncSetAttribute(k_step2d_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)local_smem_bytes());
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_step2d_local, LOC_NT, local_smem_bytes());
+            if (e == cudaSuccess) e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e == cudaSuccess && per_sm >= 1 && sms >= 1) { c->local_ok = true; c->loc_resident = per_sm * sms; }
+            cudaGetLastError();
+        }
+    }
     if (c->chunked) {
         cudaError_t e = cudaMalloc((void **)&c->dW, sizeof(double) * 4 * CH_MAX_P);
         if (e == cudaSuccess) e = cudaMemcpy(c->dW, c->fac.W, sizeof(double) * 4 * CH_MAX_P, cudaMemcpyHostToDevice);
@@ -348,9 +371,8 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         if (e == cudaSuccess) e = cudaMemcpy(c->dS2 + 128, c->fac.WG, sizeof(double) * 16, cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
             std::string msg = std::string("ch_create: ") + cudaGetErrorString(e);
-            if (c->dW) cudaFree(c->dW);
-            if (c->dS2) cudaFree(c->dS2);
-            delete c;
+            cudaGetLastError();
+            ch_destroy(c);            // frees every table allocated so far (dW, dS2, dS2c, dW16, dS2_16)
             return fail(nullptr, e == cudaErrorMemoryAllocation ? CH_ENOMEM : CH_ECUDA, msg);
         }
     }
@@ -547,7 +569,8 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         return CH_OK;
     }
     if (!strcmp(key, "fuse")) {
-        if (value < 0 || value > 4) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line) or 4 (cluster line)");
+        if (value < 0 || value > 5) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line), 4 (cluster line) or 5 (one-pass local)");
+        if (value == 5 && !ctx->local_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the one-pass local step needs D = 2, N % 4 == 0 and a decay reach <= 18 points (gamma dt <~ 0.012)");
         if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2 and N in {1024, 2048, 4096}");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
         if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 192, 256, 384, 512}");
@@ -575,6 +598,8 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "cline")) { *value = ctx->cline_ok ? ctx->cl_resident : 0; return CH_OK; }
     if (!strcmp(key, "line")) { *value = ctx->line_ok ? ctx->l_resident : 0; return CH_OK; }
     if (!strcmp(key, "fuse_mode")) { *value = fuse_mode(ctx); return CH_OK; }
+    if (!strcmp(key, "local")) { *value = ctx->local_ok ? ctx->loc_resident : 0; return CH_OK; }
+    if (!strcmp(key, "local_reach")) { *value = ctx->loc_H; return CH_OK; }
     return CH_EINVAL;
 }
 
@@ -842,6 +867,7 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
 static int fused_parts(const ch_ctx *c)
 {
     const int mode = fuse_mode(c);
+    if (mode == 5) return c->line_ok ? c->l_strips : c->nparts;
     return mode == 3 ? c->l_strips : (mode == 4 ? c->nparts : c->f_strips * c->f_CS);
 }
 
@@ -849,6 +875,12 @@ static int fused_parts(const ch_ctx *c)
 // Returns true when w is left WITHOUT the RHS scale dt / c0^2 (k_sweep_x_update then applies it).
 static bool launch_rhs_sweep_y(ch_ctx *c, bool diag, bool write)
 {
+    if (fuse_mode(c) == 5) {
+        // one-pass local step: this entry only serves its sampling reduction (diagnostics-only launch)
+        if (diag && c->line_ok) { ProfScope ps(c, KIND_RHS_SWEEP_Y_DIAG); launch_rhs_sweep_y_line(c, true, false); }
+        else if (diag) launch_rhs(c, c->C, c->w, c->rscale, true, false);
+        return true;
+    }
     if (fuse_mode(c) == 4) {
         // cluster line step: the sampling reduction is a diagnostics-only launch of the tile RHS kernel
         // (reads C once more on the 1-in-stride sampling steps), the step itself never changes kernel
@@ -907,6 +939,28 @@ static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
     else k_sweep_x_update<32><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
 }
 
+// the whole 2D step in one pass (ch_local2d.cuh): reads c->C, writes c->w, then the two arrays swap roles
+static void launch_step_local(ch_ctx *c)
+{
+    ProfScope ps(c, KIND_STEP_LOCAL);
+    LocalParams p;
+    p.np = c->fac.np; p.nq = c->fac.nq; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0; p.oscale = c->rscale;
+    p.N = c->N; p.M = c->M; p.H = c->loc_H;
+    const int He = (p.H + 1) & ~1;
+    const int swmax = (LOC_RW - 2 * He) & ~3;                  // produced columns a strip can hold, multiple of 4
+    p.nstrips = (c->N + swmax - 1) / swmax;
+    p.SW = (((c->N + p.nstrips - 1) / p.nstrips) + 3) & ~3;
+    p.total_rows = (long long)c->M * p.nstrips * c->N;
+    long long grid = c->loc_resident;
+    const long long min_span = 128;                            // a segment costs 2 H + 4 extra rows: keep spans long
+    if (grid * min_span > p.total_rows) grid = (p.total_rows + min_span - 1) / min_span;
+    if (grid < 1) grid = 1;
+    p.span = (p.total_rows + grid - 1) / grid;
+    grid = (p.total_rows + p.span - 1) / p.span;
+    k_step2d_local<<<(unsigned)grid, LOC_NT, local_smem_bytes(), c->stream>>>(p, c->C, c->w);
+    double *t = c->C; c->C = c->w; c->w = t;
+}
+
 static int check_launch(ch_ctx *ctx, const char *what)
 {
     cudaError_t e = cudaGetLastError();
@@ -920,6 +974,15 @@ static void launch_one_step(ch_ctx *ctx, bool sample)
     const int D = ctx->D;
     const bool fused = use_fused(ctx);
     bool unscaled = false;
+    if (fuse_mode(ctx) == 5) {
+        if (sample) {
+            const int np_ = launch_diag_only(ctx);
+            launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt, np_);
+            ctx->cursor++; ctx->last_sampled = ctx->n;
+        }
+        launch_step_local(ctx);
+        return;
+    }
     if (fused) unscaled = launch_rhs_sweep_y(ctx, sample, true);
     else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
     if (sample) {
@@ -960,6 +1023,7 @@ static bool ensure_graph(ch_ctx *c)
     cudaStream_t user = c->stream;
     const long long l0 = c->launches;
     const int dir0 = c->dir3;
+    double *const C0 = c->C, *const w0 = c->w;       // the local step ping-pongs them: an even number of steps restores them
     cudaGraph_t g = nullptr;
     c->stream = c->cap_stream;
     cudaError_t e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
@@ -968,6 +1032,7 @@ static bool ensure_graph(ch_ctx *c)
         e = cudaStreamEndCapture(c->cap_stream, &g);
     }
     c->stream = user; c->glaunches = c->launches - l0; c->launches = l0; c->dir3 = dir0;
+    if (c->C != C0 || c->w != w0) { c->C = C0; c->w = w0; e = e == cudaSuccess ? cudaErrorUnknown : e; }
     if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec, g, 0);
     if (g) cudaGraphDestroy(g);
     if (e != cudaSuccess) { cudaGetLastError(); c->gexec = nullptr; c->graph_broken = true; return false; }

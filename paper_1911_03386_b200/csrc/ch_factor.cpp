@@ -142,3 +142,28 @@ int ch_factor_groups(const ChFactor *f, int groups, double WG[8][4])
     }
     return 0;
 }
+
+int ch_factor_reach(const ChFactor *f, double eps, int hmax)
+{
+    // |h_k| summed far enough that the remainder is below 1e-40 of the total (rho < 1)
+    const int KMAX = 4096;
+    static thread_local ld habs[KMAX];
+    ld h1 = 1, h2 = 0, G = 0;
+    int n = 0;
+    for (; n < KMAX; ++n) {
+        habs[n] = fabsl(h1);
+        G += habs[n];
+        const ld h = (ld)f->np * h1 + (ld)f->nq * h2;
+        h2 = h1; h1 = h;
+        if (n > 8 && habs[n] < 1e-40L * G && fabsl(h1) < 1e-40L * G) { ++n; break; }
+    }
+    if (n == KMAX) return -1;                     // no decay to speak of (large gamma dt)
+    ld T = 0;
+    int H = -1;
+    for (int k = n - 1; k >= 0; --k) {            // T(k) = sum_{j >= k} |h_j|
+        T += habs[k];
+        if (2 * G * T / (ld)f->c0 > (ld)eps) { H = k + 1; break; }
+    }
+    if (H < 0) H = 0;
+    return H <= hmax ? H : -1;
+}

@@ -50,3 +50,9 @@ int ch_factor_build(ChFactor *f, int N, double sigma, int LC);
 // WG[q] = (M^32)^q (I - (M^32)^groups)^-1, q = 0..7, for a line of `groups` groups of 32 chunks of f->LC points
 // (the two-level closure across the CTAs of a cluster, ch_cline2d.cuh).  Returns 0, or -1 on bad arguments.
 int ch_factor_groups(const ChFactor *f, int groups, double WG[8][4]);
+
+// Decay reach of the factor recurrences (one-pass local step, ch_local2d.cuh): the smallest H such that a forward and a
+// backward recurrence each started from a ZERO state H points before the first point that is used reproduce
+// w = A^-1 b to within  eps * max|b|:   2 G T(H) / c0 <= eps,   h_0 = 1, h_1 = np, h_k = np h_{k-1} + nq h_{k-2}
+// (impulse response of L^-1), G = sum_k |h_k|, T(H) = sum_{k >= H} |h_k|.  Returns H, or -1 if it exceeds hmax.
+int ch_factor_reach(const ChFactor *f, double eps, int hmax);

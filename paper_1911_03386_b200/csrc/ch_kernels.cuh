@@ -259,7 +259,12 @@ __device__ __forceinline__ void chunk_state_scan(const SweepParams &prm, double 
                                                  double &a, double &b)
 {
     const int P = prm.P;
-    const unsigned full = __activemask();     // every thread of the CTA gets here together; the last warp may be partial
+    // every thread of the CTA gets here together; the last warp may be partial: the mask comes from the launch
+    // geometry, not from whichever threads happen to be converged (independent thread scheduling)
+    const unsigned nthr = blockDim.x * blockDim.y * blockDim.z;
+    const unsigned ltid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const unsigned left = nthr - (ltid & ~31u);
+    const unsigned full = left >= 32u ? 0xffffffffu : ((1u << left) - 1u);
     double ta = oa, tb = ob;
     for (int k = 0; k < prm.scan; ++k) {
         const int src = (c - dir * (1 << k)) & (P - 1);
