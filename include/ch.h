@@ -42,7 +42,9 @@
  * CH_ECUDA.
  *
  * Determinism: same inputs give bitwise-same outputs run to run; the result of a
- * member does not depend on the ensemble size or on its position in the ensemble.
+ * member does not depend on the ensemble size or on its position in the ensemble
+ * (bitwise for the exact kernels; to within the stated truncation, < 2^-56 of the
+ * local max |w| per sweep, for the one-pass local step, option "fuse" = 5).
  */
 #ifndef CH_H
 #define CH_H

@@ -95,12 +95,13 @@ struct ch_ctx {
 // which fused 2D step runs: 0 none (three-pass), 2 st.async cluster kernel, 3 line kernel, 4 cluster line kernel
 // (mode 4 steps with the cluster line kernel and samples with the tile RHS kernel), 5 one-pass local step (small
 // gamma dt only; samples with the line kernel's or the tile kernel's diagnostics-only launch)
-#define CH_LOCAL_AUTO_MIN_N 256
 static int fuse_mode(const ch_ctx *c)
 {
     if (c->opt_fuse == 1 || c->opt_sweep == 1) return 0;
     if (c->opt_fuse == 5) return c->local_ok ? 5 : 0;
-    if (c->opt_fuse == 0 && c->local_ok && c->N >= CH_LOCAL_AUTO_MIN_N) return 5;
+    // auto: the line kernels where the shape has one (measured faster: CFG3 0.218 vs 0.263 ms); everywhere else the
+    // one-pass local step when gamma dt allows it (N = 768: 0.274 vs 0.324 ms; N % 16 != 0: 0.25 vs 2.5 - 6.3 ms)
+    if (c->opt_fuse == 0 && c->local_ok && !c->line_ok && !c->cline_ok) return 5;
     if (c->opt_fuse == 2) return c->fused_ok ? 2 : 0;
     if (c->opt_fuse == 3) return c->line_ok ? 3 : 0;
     if (c->opt_fuse == 4) return c->cline_ok ? 4 : 0;
@@ -350,7 +351,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     c->line_ok = line_geometry(N, D, &c->l_strips);
     // one-pass local step: needs the decay reach of the recurrences within LOC_HMAX (gamma dt <~ 0.012)
     c->local_ok = false; c->loc_H = -1; c->loc_resident = 0;
-    if (D == 2 && N % 4 == 0 && N >= 16) {
+    if (D == 2 && N % 4 == 0 && N >= 64) {
         c->loc_H = ch_factor_reach(&c->fac, ldexp(1.0, -56), LOC_HMAX);
         if (c->loc_H >= 0) {
             if (c->loc_H < 2) c->loc_H = 2;
@@ -946,6 +947,14 @@ static void launch_step_local(ch_ctx *c)
     LocalParams p;
     p.np = c->fac.np; p.nq = c->fac.nq; p.mgam = -c->gamma; p.k1 = 4.0 * c->gamma - 1.0; p.oscale = c->rscale;
     p.N = c->N; p.M = c->M; p.H = c->loc_H;
+    {   // homogeneous solutions of the recurrence (the same numbers as ChFactor::alpha / beta, to LOC_KC entries)
+        long double a1 = 1, a2 = 0, b1 = 0, b2 = 1;
+        for (int k = 0; k < LOC_KC; ++k) {
+            const long double a = (long double)p.np * a1 + (long double)p.nq * a2, b = (long double)p.np * b1 + (long double)p.nq * b2;
+            p.al[k] = (double)a; p.be[k] = (double)b;
+            a2 = a1; a1 = a; b2 = b1; b1 = b;
+        }
+    }
     const int He = (p.H + 1) & ~1;
     const int swmax = (LOC_RW - 2 * He) & ~3;                  // produced columns a strip can hold, multiple of 4
     p.nstrips = (c->N + swmax - 1) / swmax;

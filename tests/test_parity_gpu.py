@@ -383,6 +383,122 @@ def test_flag_synchronised_kernels_are_deterministic_and_match_three_pass(B, M, 
     assert_series_close(sa, sc, 1e-12)
 
 
+# ------------------------------------- one-pass local step (option fuse = 5)
+def reach_bound(sigma, eps=2.0 ** -56):
+    """Independent restatement of the host bound (include/ch.h "local_reach"): smallest H with 2 G T(H) / c0 <= eps
+    for the causal factor 1 + p z^-1 + q z^-2 of the symbol of A = I + sigma (delta^2)^2 (roots z, conj z inside the
+    unit circle, z + 1/z = 2 + i / sqrt(sigma))."""
+    w = 2 + 1j / np.sqrt(sigma)
+    z = min((w + np.sqrt(w * w - 4)) / 2, (w - np.sqrt(w * w - 4)) / 2, key=abs)
+    p, q = -2 * z.real, abs(z) ** 2
+    c0 = sigma / q
+    h = [1.0, -p]
+    while abs(h[-1]) > 1e-40 or len(h) < 16:
+        h.append(-p * h[-1] - q * h[-2])
+    h = np.abs(np.array(h))
+    G, tails = h.sum(), np.cumsum(h[::-1])[::-1]
+    return int(np.argmax(2 * G * tails / c0 <= eps))
+
+
+def test_local_step_is_selected_from_gamma_dt_with_a_host_bound(B):
+    """The one-pass step is legal only while the factor recurrences decay within 18 points to below 2^-56 of the data;
+    the library computes that reach on the host, picks the step for shapes without a line kernel, and falls back to the
+    exact kernels otherwise (sigma = 529 must never take it)."""
+    for sigma, legal in [(0.001, True), (0.005, True), (0.01, True), (0.02, False), (1.0, False), (529.0, False)]:
+        e = B.Ensemble(1, 500, 2, sigma / 0.5, 0.5)
+        H, mode = B.ch_get_option(e.ctx, "local_reach"), B.ch_get_option(e.ctx, "fuse_mode")
+        assert (H >= 0) == legal and (mode == 5) == legal, (sigma, H, mode)
+        if legal:
+            assert H == max(2, reach_bound(sigma)), (sigma, H, reach_bound(sigma))
+        else:
+            with pytest.raises(B.ChError):
+                B.ch_set_option(e.ctx, "fuse", 5)
+        e.close()
+    for N, want in [(512, 3), (2048, 4), (768, 5), (1000, 5), (320, 5), (100, 5), (24, 0)]:
+        e = B.Ensemble(1, N, 2, 1.0, 0.01)
+        assert B.ch_get_option(e.ctx, "fuse_mode") == want, N
+        e.close()
+    e = B.Ensemble(1, 32, 3, 1.0, 0.01)                      # 3D: never
+    assert B.ch_get_option(e.ctx, "local") == 0
+    e.close()
+
+
+@pytest.mark.parametrize("name,members,nsteps", [("cfg1", [0], 1000), ("cfg2", [0, 31, 63], 1000), ("cfg3", [0, 77, 127], 1000)])
+def test_local_step_parity_1000_steps(B, oracle, name, members, nsteps):
+    """north_star bar on the one-pass step: cfg1, cfg2 and cfg3 (full ensembles on the GPU, member subsets on the
+    oracle), 1000 steps, field 1e-10, series 1e-9."""
+    c = inputs.CONFIGS[name]
+    C0 = inputs.config_state(name)
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], nsteps, c["stride"], options={"fuse": 5})
+    Co, so = oracle.run(C0[members], c["gamma"], c["dt"], nsteps, c["stride"])
+    assert np.abs(C[members] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, members], so)
+    mass = s[:, :, 3]
+    assert np.abs(mass - mass[0]).max() <= 1e-9 * max(np.abs(mass[0]).max(), 1.0)
+
+
+@pytest.mark.parametrize("M,N,nsteps,gamma,dt", [
+    (3, 100, 300, 1.0, 0.01),        # N % 16 != 0: strips narrower than a CTA, idle warps, tile-kernel sampling
+    (2, 68, 200, 1.0, 0.01),         # the C window of a strip wraps around the whole member
+    (1, 500, 200, 1.0, 0.01),        # three ragged strips (168, 168, 164 columns)
+    (1, 1000, 100, 0.5, 0.01),       # reach 15
+    (5, 768, 60, 1.0, 0.01),         # spans that cut strips and members at arbitrary rows
+    (2, 1536, 40, 2.0, 0.005),
+    (37, 256, 50, 1.0, 0.01),        # more segments than CTAs: several segments per CTA
+    (1, 2048, 30, 1.0, 0.001),       # reach 12: different geometry (wider strips)
+])
+def test_local_step_shapes(B, oracle, M, N, nsteps, gamma, dt):
+    C0 = inputs.initial_state(range(900, 900 + M), N, 2, [(-0.4, 0.0, 0.3)[k % 3] for k in range(M)], 0.2)
+    C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options={"fuse": 5})
+    sub = sorted({0, M // 2, M - 1})
+    Co, so = oracle.run(C0[sub], gamma, dt, nsteps, 10)
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
+    if M > 3:                         # every member against the exact two-kernel / three-pass step
+        R, sr = run_gpu(B, C0, gamma, dt, nsteps, 10, options={"fuse": 1})
+        assert np.abs(C - R).max() <= 1e-13
+        assert_series_close(s, sr, 1e-12)
+
+
+@pytest.mark.parametrize("M,N,steps", [(128, 512, 12), (9, 1000, 8), (3, 2048, 6), (74, 320, 16)])
+def test_local_step_is_deterministic(B, M, N, steps):
+    """Warps of the one-pass kernel synchronise through per-warp mbarriers and three CTA barriers per block and drift
+    apart in between: 20 repeats, half of them with a second stream keeping the GPU busy, must agree bitwise."""
+    import torch
+    C0 = torch.from_numpy(inputs.initial_state(range(300, 300 + M), N, 2, -0.3, 0.1)).cuda()
+    side, junk = torch.cuda.Stream(), torch.empty(32 << 20, dtype=torch.float32, device="cuda")
+    e = B.Ensemble(M, N, 2, 1.0, 0.01, options={"fuse": 5})
+    ref = None
+    for rep in range(20):
+        e.set_state(C0)
+        if rep % 2:
+            with torch.cuda.stream(side):
+                for _ in range(10):
+                    junk.mul_(1.0001)
+        e.step(steps)
+        out = torch.empty_like(C0)
+        B.ch_get_state(e.ctx, out)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(out).all())
+        if ref is None:
+            ref = out
+        else:
+            assert bool((out == ref).all()), rep
+    e.close()
+
+
+def test_local_step_member_independence_and_graph(B):
+    C0 = inputs.initial_state(range(40, 47), 320, 2, -0.2, 0.1)
+    a, sa = run_gpu(B, C0, 1.0, 0.01, 64, 16, options={"fuse": 5, "graph": 1})
+    g, sg = run_gpu(B, C0, 1.0, 0.01, 64, 16, options={"fuse": 5, "graph": 2})
+    assert np.array_equal(a, g) and np.array_equal(sa, sg)             # CUDA graph of 8 ping-pong steps
+    # a member's result does not depend on the ensemble around it -- up to the truncation (< 2^-56 of the local max |w|
+    # per sweep): where the CTA spans cut the strips depends on the ensemble size, so this is round-off, not bitwise
+    one, s1 = run_gpu(B, C0[4:5].copy(), 1.0, 0.01, 64, 16, options={"fuse": 5})
+    assert np.abs(one[0] - a[4]).max() <= 1e-15
+    assert_series_close(s1[:, :1], sa[:, 4:5], 1e-13)
+
+
 def test_equivariances_on_gpu(B):
     C0 = inputs.initial_state([3, 4], 128, 2, [0.0, -0.3], 0.2)
     base, _ = run_gpu(B, C0, 1.0, 0.01, 50, 50)
