@@ -194,6 +194,38 @@ int ch_grid_doubling_error(const double *fine_dev, const double *coarse_dev, int
 /* Message for the last error on this context (never NULL); ch_create failures: pass NULL. */
 const char *ch_last_error(const ch_ctx *ctx);
 
+/* ---- Model 1: ensembles of droplet populations (off the hot path) ----
+ * `realisations` independent populations of N droplets each (the paper: M = 100, N = 128 ... 8192, Table 1),
+ *     dR_i/dt = H(R_i + eps) (-1/R_i^2 + ubar/R_i),   ubar = sum_i H(R_i) / sum_i H(R_i) R_i     eq. (39), eq. (14)
+ * (H(s) = 1 for s > 0, else 0; eps = 1e-3 in the paper), integrated with the Dormand-Prince 5(4) pair -- the method of the
+ * paper's ODE45, P:368 -- one CTA per realisation, the whole time loop in one launch.  Step controller (the paper states
+ * none; reading G21): err = max_i |e_i| / (atol + rtol max(|R_i|, |R_i^new|)), accept iff err <= 1,
+ * h_new = h min(5, max(0.2, 0.9 err^(-1/5))), the step clipped to land on t_end.
+ * Layout: R[realisation][droplet], contiguous doubles.  Every call is asynchronous on the context's stream unless it
+ * copies to or from host memory.  Errors as above (CH_EINVAL, CH_ENOMEM, CH_ECUDA, CH_ESTATE).
+ *
+ * ch_droplet_set_state: copies realisations * N radii in and resets every realisation's time to 0.
+ * ch_droplet_integrate: advance every realisation from its current time to t_end (at most max_steps attempted steps,
+ *   first trial step h0).  steps_dev (may be NULL): device double[realisations][max_record], receives the ACCEPTED step
+ *   sizes; nsteps_dev (may be NULL): device int[realisations], their number.
+ * ch_droplet_replay: advance by GIVEN step sizes without error control: steps_dev is device double[realisations][stride],
+ *   the first nsteps entries of a row are used, a non-positive entry ends the row early.  (With the step sequence of a
+ *   reference integration this reproduces it to round-off: the parity test.)
+ * ch_droplet_energy: out[realisations][4] = {F, dF/dt, beta, V} at each realisation's current time t:
+ *   F = sum_i H(R_i) R_i^2 / 2 (eq. (31)), dF/dt = -sum_i H(R_i) (1 - ubar R_i)^2 / R_i (eq. (33)),
+ *   beta = -(t/F) dF/dt (eq. (36)), V = sum_i H(R_i) R_i^3 / 3 (the conserved volume). */
+typedef struct ch_droplet_ctx ch_droplet_ctx;
+int ch_droplet_create(ch_droplet_ctx **out, int realisations, int N, double eps);
+int ch_droplet_destroy(ch_droplet_ctx *ctx);
+int ch_droplet_set_stream(ch_droplet_ctx *ctx, void *cuda_stream);
+int ch_droplet_set_state(ch_droplet_ctx *ctx, const double *R, int on_device);
+int ch_droplet_get_state(ch_droplet_ctx *ctx, double *R, int on_device);
+int ch_droplet_integrate(ch_droplet_ctx *ctx, double t_end, double rtol, double atol, double h0, long long max_steps,
+                         double *steps_dev, int max_record, int *nsteps_dev);
+int ch_droplet_replay(ch_droplet_ctx *ctx, const double *steps_dev, int nsteps, int stride);
+int ch_droplet_energy(ch_droplet_ctx *ctx, double *out, int on_device);
+const char *ch_droplet_last_error(const ch_droplet_ctx *ctx);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,6 +19,8 @@ EXPORTS = [
     "ch_create", "ch_destroy", "ch_set_stream", "ch_workspace_bytes", "ch_attach_workspace",
     "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_energy", "ch_get_state",
     "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
+    "ch_droplet_create", "ch_droplet_destroy", "ch_droplet_set_stream", "ch_droplet_set_state", "ch_droplet_get_state",
+    "ch_droplet_integrate", "ch_droplet_replay", "ch_droplet_energy", "ch_droplet_last_error",
     "ch_launch_count", "ch_last_error", "ch_profile", "ch_profile_read", "ch_kernel_kinds",
     "ch_kernel_kind_name", "ch_stats_moments", "ch_stats_hist", "ch_stats_fit", "ch_grid_doubling_error",
 ]
@@ -74,6 +76,16 @@ def lib():
         L.ch_grid_doubling_error.argtypes = [dp, dp, ci, ci, dp, vp]
         L.ch_last_error.argtypes = [vp]
         L.ch_last_error.restype = ctypes.c_char_p
+        L.ch_droplet_create.argtypes = [ctypes.POINTER(vp), ci, ci, cd]
+        L.ch_droplet_destroy.argtypes = [vp]
+        L.ch_droplet_set_stream.argtypes = [vp, vp]
+        L.ch_droplet_set_state.argtypes = [vp, dp, ci]
+        L.ch_droplet_get_state.argtypes = [vp, dp, ci]
+        L.ch_droplet_integrate.argtypes = [vp, cd, cd, cd, cd, ctypes.c_longlong, dp, ci, vp]
+        L.ch_droplet_replay.argtypes = [vp, dp, ci, ci]
+        L.ch_droplet_energy.argtypes = [vp, dp, ci]
+        L.ch_droplet_last_error.argtypes = [vp]
+        L.ch_droplet_last_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -225,6 +237,56 @@ def ch_grid_doubling_error(fine, coarse, out, stream=None):
     assert tuple(fine.shape) == (M, 2 * n, 2 * n) and tuple(coarse.shape) == (M, n, n) and out.numel() == M
     _stats_check(lib().ch_grid_doubling_error(fine.data_ptr(), coarse.data_ptr(), M, n, out.data_ptr(),
                                               ctypes.c_void_p(stream or 0)), "ch_grid_doubling_error")
+
+
+# ---- Model 1: droplet populations (include/ch.h, ch_droplet_*) ---------------------------
+def _dcheck(ctx, rc):
+    if rc != CH_OK:
+        raise ChError(rc, lib().ch_droplet_last_error(ctx).decode())
+
+
+def ch_droplet_create(realisations, N, eps):
+    ctx = ctypes.c_void_p()
+    rc = lib().ch_droplet_create(ctypes.byref(ctx), realisations, N, eps)
+    if rc != CH_OK:
+        raise ChError(rc, lib().ch_droplet_last_error(None).decode())
+    return ctx
+
+
+def ch_droplet_destroy(ctx):
+    return lib().ch_droplet_destroy(ctx)
+
+
+def ch_droplet_set_stream(ctx, stream):
+    _dcheck(ctx, lib().ch_droplet_set_stream(ctx, ctypes.c_void_p(stream)))
+
+
+def ch_droplet_set_state(ctx, R):
+    p, dev = _ptr(R)
+    _dcheck(ctx, lib().ch_droplet_set_state(ctx, p, dev))
+
+
+def ch_droplet_get_state(ctx, R):
+    p, dev = _ptr(R)
+    _dcheck(ctx, lib().ch_droplet_get_state(ctx, p, dev))
+
+
+def ch_droplet_integrate(ctx, t_end, rtol=1e-6, atol=1e-9, h0=1e-4, max_steps=10_000_000, steps=None, nsteps=None):
+    """steps: CUDA float64 tensor [M][max_record] or None; nsteps: CUDA int32 tensor [M] or None (outputs)."""
+    _dcheck(ctx, lib().ch_droplet_integrate(ctx, t_end, rtol, atol, h0, max_steps,
+                                            None if steps is None else steps.data_ptr(), 0 if steps is None else steps.shape[1],
+                                            None if nsteps is None else nsteps.data_ptr()))
+
+
+def ch_droplet_replay(ctx, steps):
+    """steps: CUDA float64 tensor [M][nsteps]; a non-positive entry ends a row early."""
+    assert steps.is_cuda and steps.is_contiguous()
+    _dcheck(ctx, lib().ch_droplet_replay(ctx, steps.data_ptr(), steps.shape[1], steps.shape[1]))
+
+
+def ch_droplet_energy(ctx, out):
+    p, dev = _ptr(out)
+    _dcheck(ctx, lib().ch_droplet_energy(ctx, p, dev))
 
 
 # ---- convenience wrapper ---------------------------------------------------------------

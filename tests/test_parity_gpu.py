@@ -166,12 +166,13 @@ def test_cfg3_headline_config_member_subset(B, oracle):
 
 
 def test_cfg4_3d_member_subset(B, oracle):
-    """configs[3] at full size (16 x 128^3); the oracle follows one member of each mixture for 100 steps."""
+    """configs[3] at full size (16 x 128^3, the production 3D kernels: z-marching RHS, plane-pair x/y sweeps, fused
+    z-sweep); north_star depth: the oracle follows one member of each mixture for 1000 steps (~90 s of host time)."""
     c = inputs.CONFIGS["cfg4"]
     C0 = inputs.config_state("cfg4")
-    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 100, c["stride"])
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 1000, c["stride"])
     sub = [0, 15]
-    Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 100, c["stride"])
+    Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 1000, c["stride"])
     assert np.abs(C[sub] - Co).max() <= FIELD_TOL
     assert_series_close(s[:, sub], so)
 
@@ -207,8 +208,8 @@ def test_3d_plane_sweep_paper_regime(B, oracle):
         Co, so = oracle.run(C0, 66.4, 7.97, nsteps, 2)
         for opts in (None, {"sweep3": 2}):               # N = 128: cluster pair / one CTA per plane
             C, s = run_gpu(B, C0, 66.4, 7.97, nsteps, 2, options=opts)
-            assert np.abs(C - Co).max() <= 1e-9, (N, opts)
-            assert_series_close(s, so, 1e-7)
+            assert np.abs(C - Co).max() <= FIELD_TOL, (N, opts)       # measured <= 1.5e-13
+            assert_series_close(s, so)
 
 
 def test_small_3d_1000_steps(B, oracle):
@@ -219,25 +220,27 @@ def test_small_3d_1000_steps(B, oracle):
     assert_series_close(s, so)
 
 
-def test_cfg5_long_lines_one_member(B, oracle):
-    """configs[4] at full size (8 x 2048^2); the oracle follows one member for 50 steps."""
+def test_cfg5_long_lines_two_members(B, oracle):
+    """configs[4] at full size (8 x 2048^2, cluster line kernel of 4 CTAs per line); north_star depth: the oracle
+    follows two members for 1000 steps (~3 min of host time, side by side)."""
     c = inputs.CONFIGS["cfg5"]
     C0 = inputs.config_state("cfg5")
-    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 50, c["stride"])
-    Co, so = oracle.run(C0[[5]], c["gamma"], c["dt"], 50, c["stride"])
-    assert np.abs(C[[5]] - Co).max() <= FIELD_TOL
-    assert_series_close(s[:, [5]], so)
+    C, s = run_gpu(B, C0, c["gamma"], c["dt"], 1000, c["stride"])
+    sub = [2, 5]
+    Co, so = oracle.run(C0[sub], c["gamma"], c["dt"], 1000, c["stride"])
+    assert np.abs(C[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, sub], so)
 
 
 def test_4096_lines_cluster_of_eight(B, oracle):
     """The paper's largest grid (n = 4096): cluster line kernel with 8 CTAs per line, sampling through
-    the tile RHS kernel; one member, 6 steps sampled every 3, against the oracle."""
+    the tile RHS kernel; one member, 100 steps sampled every 25, against the oracle (~70 s of host time)."""
     C0 = inputs.initial_state([4242], 4096, 2, -0.2, 0.05)
     e = B.Ensemble(1, 4096, 2, 1.0, 0.01)
     assert B.ch_get_option(e.ctx, "fuse_mode") == 4
     e.close()
-    C, s = run_gpu(B, C0, 1.0, 0.01, 6, 3)
-    Co, so = oracle.run(C0, 1.0, 0.01, 6, 3)
+    C, s = run_gpu(B, C0, 1.0, 0.01, 100, 25)
+    Co, so = oracle.run(C0, 1.0, 0.01, 100, 25)
     assert np.abs(C - Co).max() <= FIELD_TOL
     assert_series_close(s, so)
 
@@ -284,8 +287,30 @@ def test_paper_regime_large_sigma(B, oracle):
     C0 = inputs.initial_state([7, 8], 128, 2, [0.0, -0.4], 0.05)
     C, s = run_gpu(B, C0, 66.4, 7.97, 200, 10)
     Co, so = oracle.run(C0, 66.4, 7.97, 200, 10)
-    assert np.abs(C - Co).max() <= 1e-9
-    assert_series_close(s, so, 1e-7)
+    # two oracle formulations (banded + Schur vs dense pivoted) differ by 5.6e-12 after these 200
+    # steps at 64^2, the GPU differs from the oracle by 5.8e-12: the north star's bar holds at cond(A) = 8.5e3 too
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+
+
+@pytest.mark.parametrize("N,M", [(512, 2), (1024, 1), (2048, 1), (4096, 1)])
+def test_sweeps_at_the_convergence_study_extreme(B, oracle, N, M):
+    """gamma dt / dx^4 = 2.77e5 (Appendix A at n = 4096; cond(A) = 4.4e6 per factor): every sweep variant the
+    grid-doubling study runs (chunked LU with the two-level scan closure, K-term sum, generic) against the oracle's
+    banded solve.  Measured 2.3e-11 relative = 0.05 cond(A) eps; bar = 0.5 cond(A) eps."""
+    sigma = 2.77e5
+    rng = np.random.default_rng(N)
+    w = rng.standard_normal((M, N, N))
+    tol = 0.5 * (1 + 16 * sigma) * 2.0 ** -53
+    e = B.Ensemble(M, N, 2, sigma / 0.5, 0.5)
+    ref = [oracle.sweep(w, sigma, axis) for axis in (0, 1)]
+    for opts in ({}, {"scan": 1}, {"scan": 2}, {"sweep": 1}):
+        for k, v in {"scan": 0, "sweep": 0, **opts}.items():
+            B.ch_set_option(e.ctx, k, v)
+        for axis in (0, 1):
+            got = e.sweep(w, axis)
+            assert np.abs(got - ref[axis]).max() <= tol * np.abs(ref[axis]).max(), (opts, axis)
+    e.close()
 
 
 def test_generic_paths_end_to_end(B, oracle):
@@ -308,16 +333,17 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     nsteps = 100 if N <= 256 else 20
     C0 = inputs.initial_state([5, 6][:M], N, 2, [0.0, -0.4][:M], 0.1)
     Co, so = oracle.run(C0, gamma, dt, nsteps, 10)
-    tol, rtol = (FIELD_TOL, SERIES_RTOL) if gamma == 1.0 else (1e-9, 1e-7)
+    tol, rtol = FIELD_TOL, SERIES_RTOL                      # also at gamma dt = 529
     e = B.Ensemble(M, N, 2, gamma, dt)
     cs, line, mode = B.ch_get_option(e.ctx, "fused"), B.ch_get_option(e.ctx, "line"), B.ch_get_option(e.ctx, "fuse_mode")
-    cline = B.ch_get_option(e.ctx, "cline")
+    cline, local = B.ch_get_option(e.ctx, "cline"), B.ch_get_option(e.ctx, "local")
     e.close()
+    assert (local != 0) == (gamma == 1.0 and N >= 64)          # one-pass local step: small gamma dt only
     assert (cs == 0) == (N == 592)
     assert (line != 0) == (N in (32, 64, 96, 128, 192, 256, 384, 512))
     assert (cline != 0) == (N == 1024)                         # flag kernel at K <= 2, scan kernel in the paper regime
-    assert mode == (3 if line else (4 if cline else (2 if cs else 0)))
-    variants = [{"fuse": 1}] + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
+    assert mode == (3 if line else (4 if cline else (5 if local else (2 if cs else 0))))
+    variants = [{"fuse": 1}] + ([{"fuse": 5}] if local else []) + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
         + ([{"fuse": 4}] if cline else [])
     for opts in variants:
         C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options=opts)
@@ -497,6 +523,44 @@ def test_local_step_member_independence_and_graph(B):
     one, s1 = run_gpu(B, C0[4:5].copy(), 1.0, 0.01, 64, 16, options={"fuse": 5})
     assert np.abs(one[0] - a[4]).max() <= 1e-15
     assert_series_close(s1[:, :1], sa[:, 4:5], 1e-13)
+
+
+@pytest.mark.parametrize("M,N,steps", [
+    (7, 512, 12), (8, 512, 12), (9, 512, 12), (16, 512, 8), (17, 512, 8), (41, 512, 6),     # 130, 148, 167, 296, 315, 759 tiles on 148 CTAs
+    (33, 256, 10), (75, 128, 10),                                                           # two line-kernel CTAs per SM
+    (3, 1024, 8), (5, 1024, 6), (2, 2048, 6), (3, 2048, 5), (1, 4096, 4),                    # clusters of 2, 4, 8 CTAs per line
+])
+def test_flag_synchronised_kernels_repeat_bitwise_under_load(B, M, N, steps):
+    """compute-sanitizer is closed on this pool, so the hand-rolled release/acquire protocols of the line kernel
+    (per-warp sequence flags, single-buffered slots, packed leftover tiles for odd M) and of the cluster line kernel
+    (st.release.cluster / ld.acquire.cluster ghost slots) are exercised instead: 20 repeats per shape -- tile counts
+    just below, at and just above multiples of the 148 resident CTAs, odd ensembles -- every other one with a second
+    stream keeping the SMs busy so that CTA scheduling and warp drift vary; all must agree bitwise."""
+    import torch
+    C0 = torch.from_numpy(inputs.initial_state(range(700, 700 + M), N, 2, -0.3, 0.1)).cuda()
+    side, junk = torch.cuda.Stream(), torch.empty(32 << 20, dtype=torch.float32, device="cuda")
+    e = B.Ensemble(M, N, 2, 1.0, 0.01)
+    assert B.ch_get_option(e.ctx, "fuse_mode") in (3, 4)
+    ser = torch.empty((steps // 2 + 1, M, 4), dtype=torch.float64, device="cuda")
+    ref = None
+    for rep in range(20):
+        e.set_state(C0)
+        e.set_series(2, steps // 2 + 1)                     # sampling variants (CTA barriers) interleaved with the flag kernels
+        if rep % 2:
+            with torch.cuda.stream(side):
+                for _ in range(8):
+                    junk.mul_(1.0001)
+        e.step(steps)
+        out = torch.empty_like(C0)
+        B.ch_get_state(e.ctx, out)
+        ser.copy_(e._series)
+        torch.cuda.synchronize()
+        if ref is None:
+            ref, sref = out, ser.clone()
+            assert bool(torch.isfinite(out).all())
+        else:
+            assert bool((out == ref).all()) and bool((ser == sref).all()), rep
+    e.close()
 
 
 def test_equivariances_on_gpu(B):
