@@ -31,17 +31,19 @@ FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS
 # every kernel reads and writes one fp64 field; the last sweep also reads C^n for the fused update.
 ALGO_BYTES = {
     2: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 24,
-        "rhs_sweep_y": 16, "rhs_sweep_y_diag": 16, "sweep_x_update": 24},      # fused 2D step: 40 B per update
+        "rhs_sweep_y": 16, "rhs_sweep_y_diag": 16, "sweep_x_update": 24,       # fused 2D step: 40 B per update
+        "step_local": 16},                                                     # one-pass local step: read C^n, write C^{n+1}
     3: {"rhs": 16, "rhs_diag": 16, "sweep_x": 16, "sweep_y": 16, "sweep_z": 24, "sweep_xy": 16},   # plane kernel: x + y in one pass
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, kernel); None until captured.
+# value = (bytes per launch, the committed capture it was read from).  One launch under `ncu --set full`: caches are
+# flushed before the launch, so the L2 hits the live step gets from walking the ensemble up in one kernel and down in
+# the next do not show, and part of the write-back is still in L2 when the launch ends.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_v8_ncu_full_cfg3.md: one launch under `ncu --set full` (caches flushed before the launch, so the
-    # L2 hits the live step gets from walking the ensemble up in one kernel and down in the next do not show; part of
-    # the 268 MB write-back was still in L2 when the launch ended)
-    ("cfg3", "sweep_x_update"): 749.5e6,
-    ("cfg3", "rhs_sweep_y"): 487.9e6,
+    ("cfg3", "sweep_x_update"): (749.5e6, "profiles/r01_v8_ncu_full_cfg3.md"),
+    ("cfg3", "rhs_sweep_y"): (485.6e6, "profiles/r01_v8_ncu_full_cfg3.md"),
+    ("cfg3", "step_local"): (697.4e6, "profiles/r02_ncu_full_local.md"),
 }
 
 
@@ -178,7 +180,11 @@ def run_ours(args):
     host_out = torch.empty_like(host).pin_memory()
 
     stream = torch.cuda.current_stream()
-    ens = B.Ensemble(M, N, D, c["gamma"], c["dt"], stream=stream.cuda_stream)
+    opts = {}
+    for kv in args.option:
+        k, v = kv.split("=")
+        opts[k] = int(v)
+    ens = B.Ensemble(M, N, D, c["gamma"], c["dt"], stream=stream.cuda_stream, options=opts)
     dstate = host.to(dev, non_blocking=True)
     torch.cuda.synchronize()
 
@@ -224,6 +230,7 @@ def run_ours(args):
     repetitions = {"n": R, "ms_per_step_median": rep_ms[med] / K, "ms_per_step_min": min(rep_ms) / K,
                    "ms_per_step_max": max(rep_ms) / K, "samples_per_repetition": rep_samples}
 
+    fuse_mode_used = B.ch_get_option(ens.ctx, "fuse_mode") if D == 2 else None
     # ---- per-kernel leg: same steps with every launch bracketed by CUDA events on the stream
     B.ch_profile(ens.ctx, 1)
     ens.set_state(dstate)
@@ -246,17 +253,19 @@ def run_ours(args):
     # bytes one step must move in the pass structure that ran: fused 2D step 16 + 24 = 40 B per update
     # (DESIGN.md section 5), three-pass 2D 56 B, four-pass 3D 72 B
     fused = "sweep_x_update" in kernels
-    step_bytes = 40 if fused else (56 if D == 2 else (56 if "sweep_xy" in kernels else 72))
+    step_bytes = 16 if "step_local" in kernels else (40 if fused else (56 if D == 2 else (56 if "sweep_xy" in kernels else 72)))
     model_bytes = 56 if D == 2 else 72
     main_kinds = {k: v for k, v in kernels.items() if not k.endswith("_diag")} or kernels
     dom = max(main_kinds, key=lambda k: main_kinds[k]["avg_ms"] * main_kinds[k]["launches"])
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES.get((name, dom)),
+                "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES.get((name, dom), (None, None))[0],
+                "traffic_source": NCU_TRAFFIC_BYTES.get((name, dom), (None, None))[1],
                 "peak_source": peak_src, "share_of_step": kernels[dom]["avg_ms"] * kernels[dom]["launches"] / total_kernel_ms,
                 "step_algo_bytes_per_update": step_bytes,
                 "step_achieved_gbs": value / world * step_bytes / 1e9,
                 "step_frac": value / world * step_bytes / 1e9 / peak,
                 "step_frac_of_8TBs_nominal": value / world * step_bytes / 1e9 / 8000.0,
+                "step_frac_of_16B_floor": value / world * 16 / 1e9 / peak,      # read C^n once, write C^{n+1} once
                 "note": ("achieved = algorithmic bytes / live CUDA-event time; a fraction above 1 means part of those bytes came from L2: "
                          "consecutive kernels walk the ensemble in opposite directions, so each finds the tail of its predecessor's "
                          "output in the 126 MB L2 (the ncu `traffic` figure is taken with caches flushed per launch)"),
@@ -267,7 +276,7 @@ def run_ours(args):
     # paper's gamma = 0.01, dx = 2 pi / 512, dt = 0.0012 in h = 1 units): the closure tables do not decay
     paper_regime = None
     if args.paper_regime:
-        ens2 = B.Ensemble(M, N, D, 66.4, 7.97, stream=stream.cuda_stream)
+        ens2 = B.Ensemble(M, N, D, 66.4, 7.97, stream=stream.cuda_stream, options=opts if "fuse" not in opts else {})
         ens2.set_state(dstate)
         ens2.set_series(stride, cap)
         ens2.step(W)
@@ -316,7 +325,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": secs / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_desc(name), "members_per_gpu": M, "parallelism": f"ensemble-sharded x{world} (no data-path collective)",
+            "config": {"workload": workload_desc(name), "members_per_gpu": M, "options": opts, "fuse_mode": fuse_mode_used, "parallelism": f"ensemble-sharded x{world} (no data-path collective)",
                        "l2": f"working set {2 * state_bytes >> 20} MiB per GPU, larger than the 126 MB L2; no explicit flush",
                        "sampling": (f"F, dF/dt, beta, mass every {stride} steps; {samples_in} sampling step(s) inside the {K}-step timed region "
                                     f"(every repetition starts at step n = {phase} mod {stride})")},
@@ -338,6 +347,8 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed K-step region (median reported)")
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=INT",
+                    help="kernel-variant option passed to ch_set_option (include/ch.h), e.g. fuse=5; repeatable")
     ap.add_argument("--no-paper-regime", dest="paper_regime", action="store_false",
                     help="skip the extra timed leg at the paper's gamma dt / h^4 = 529")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (for runs under ncu)")

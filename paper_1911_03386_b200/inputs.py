@@ -57,6 +57,11 @@ CONFIGS = {
                  cbar=-0.2, amp=0.05, seed0=4000),
 }
 
+# Not BASELINE.json configs: two shapes OUTSIDE the enumerated fast-kernel sizes (N not a power of two; N % 16 != 0), the
+# cases the one-pass local step serves.  Same recipe as cfg3 (asymmetric mixture, 2^25 points).
+CONFIGS["n768"] = dict(ensemble=57, N=768, D=2, gamma=1.0, dt=0.01, nsteps=20000, stride=50, cbar=-0.4, amp=0.05, seed0=5000)
+CONFIGS["n1000"] = dict(ensemble=32, N=1000, D=2, gamma=1.0, dt=0.01, nsteps=20000, stride=50, cbar=-0.4, amp=0.05, seed0=6000)
+
 
 def config_state(name: str, members=None) -> np.ndarray:
     """Initial ensemble of a named config; `members` selects a subset of member indices."""
