@@ -4,24 +4,31 @@
 //   k_step2d_local   C^{n+1} = C^n + (dt / c0^2) Lx^-T Lx^-1 Ly^-T Ly^-1 Lap_h mu(C^n)          P:29-30, include/ch.h
 //
 // Why it is legal.  A_d = c0 L^T L with L = I + p S^-1 + q S^-2 (ch_factor.h); the impulse response h_k of L^-1 decays
-// like rho^k, rho = |root| (0.0976 at gamma dt = 0.01).  A recurrence started from a ZERO state H points before the
+// like rho^k, rho = |root| (0.0972 at gamma dt = 0.01).  A recurrence started from a ZERO state H points before the
 // first point that is used differs from the cyclic one by at most T(H) = sum_{k >= H} |h_k| times the data, and the
 // host picks the smallest H with 2 G T(H) / c0 <= 2^-56 (ch_factor_reach; G = sum |h_k|): the truncation is below an
 // eighth of an ulp of the local max |w| per sweep.  If that needs H > LOC_HMAX the exact two-kernel step runs instead.
 //
 // Structure.  The columns of a member are cut into strips of SW produced columns; a strip is computed on
-// SW + 2 H columns (r-region) from SW + 2 H + 4 columns of C.  All strips of all members, stacked row after row, form a
-// "tape"; every CTA (2 per SM, 7 warps) marches down an equal span of it, segment by segment (a segment = consecutive
-// rows of one strip; it starts H + 2 rows early and ends H + 2 rows late, rows wrap).  Per block of 32 rows:
-//   P1 (thread = column)   rows arrive by 16-byte cp.async in a 16-row ring; rolling register window: mu of the next row
-//                          (x-neighbours of C from the ring, of mu by shuffle -- the 7 warps overlap by two columns),
-//                          r = Lap_h mu, forward y-recurrence z (exact streaming, state in registers), z -> z-ring
-//   P2 (thread = column)   backward y-recurrence over the block from a zero state H rows below it (H throw-away
-//                          rows), in place: the 32 rows that are H rows behind the front are final
-//   P3 (lane = row, warp = 30-column chunk)   x-sweep of those rows in place: forward / backward recurrence over the
-//                          chunk after an H-column zero-state warm-up read from the neighbouring chunk
-//   P4 (thread = column)   C^{n+1} = C^n + scale * w, C^n re-read through L2 (it was read ~50 rows ago), coalesced
+// SW + 2 He columns (r-region, He = H rounded up to even) from SW + 2 He + 4 columns of C.  All strips of all members,
+// stacked row after row, form a "tape"; every CTA (2 per SM, 7 warps) marches down an equal span of it, segment by
+// segment (a segment = consecutive rows of one strip; it starts H + 2 rows early and ends H + 2 rows late, rows wrap).
+// Per block of 32 rows:
+//   P1 (warp w, lane l = r-region column 30 w + l - 1; lanes 1..30 produce, warps overlap by two columns)
+//        the warp stages the 34 C columns it needs itself: one cp.async.bulk per row issued by an elected lane, completion on
+//        the warp's own three mbarriers, 12-row ring, L2 prefetch LOC_PF rows ahead.  Rolling register window: mu of the
+//        next row (x-neighbours of C from the ring, of mu by shuffle), r = Lap_h mu, forward y-recurrence z (exact
+//        streaming, state in registers), z -> z-ring.  No CTA barrier: warps drift apart, load / fp64 phases overlap.
+//   P2 (same thread, its own column)   backward y-recurrence from a zero state at the newest row, H throw-away rows, in
+//        place: the 32 rows that are H behind the front are final
+//   P3 (lane = row, warp = chunk of 30 columns)   forward then backward x-recurrence of the chunk from a zero state, in
+//        place; the state entering a chunk is its neighbour's zero-state out-state (exact to rho^28), applied as
+//        alpha_k a + beta_k b to the first / last LOC_KC points: the forward correction inside the backward pass, the
+//        backward correction inside P4.  Two CTA barriers.
+//   P4 (warp = its own 30 columns, half-warp = row parity, lane = column pair)   C^{n+1} = C^n + scale (w + correction),
+//        C^n re-read through L2, 16-byte stores.  P4 and the next P1 of a warp touch the same columns: no barrier needed.
 // The result goes to a second array (the halo of a strip is another strip's interior): ch_step ping-pongs C and w.
+// Measured and bounded in profiles/r02_ncu_full_local.md (shared-memory data pipe 69 %, issue 48 %, 2 x 7 warps per SM).
 #pragma once
 
 #include <cuda_runtime.h>
