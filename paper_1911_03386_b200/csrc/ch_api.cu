@@ -201,7 +201,7 @@ static int max_parts(int N, int D)
 {
     int n = rhs_parts(N, D), cpb, cs, st;
     if (fused_geometry(N, D, &cpb, &cs, &st) && st * cs > n) n = st * cs;
-    if (line_geometry(N, D, &st) && st > n) n = st;
+    if (line_geometry(N, D, &st) && st * (N / 32) > n) n = st * (N / 32);      // one partial per (strip, warp)
     if (rhs3_stream_geometry(N, D, &st) && st > n) n = st;
     return n;
 }
@@ -404,6 +404,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
             e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);   \
             if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
             if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_sweep_y_line<NC, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
             if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_rhs_sweep_y_line<NC, false, false>, NC, smem); \
         }
         LINE_SIZES(X)
@@ -826,7 +827,8 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
     const bool nb = p.K <= 2 && c->opt_linesync != 1;     // neighbour-warp synchronisation instead of CTA barriers
 #define X(NC)                                                                                                       \
     if (c->N == NC) {                                                                                               \
-        if (diag) k_rhs_sweep_y_line<NC, true, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials);   \
+        if (diag && nb) k_rhs_sweep_y_line<NC, true, true><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
+        else if (diag) k_rhs_sweep_y_line<NC, true, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
         else if (nb) k_rhs_sweep_y_line<NC, false, true><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
         else k_rhs_sweep_y_line<NC, false, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials);       \
     }
@@ -868,8 +870,8 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
 static int fused_parts(const ch_ctx *c)
 {
     const int mode = fuse_mode(c);
-    if (mode == 5) return c->line_ok ? c->l_strips : c->nparts;
-    return mode == 3 ? c->l_strips : (mode == 4 ? c->nparts : c->f_strips * c->f_CS);
+    if (mode == 5) return c->line_ok ? c->l_strips * (c->N / 32) : c->nparts;
+    return mode == 3 ? c->l_strips * (c->N / 32) : (mode == 4 ? c->nparts : c->f_strips * c->f_CS);
 }
 
 // diag: also reduce F, Fdot, mass of C^n into the partials; write == false (diag only): no sweep, w untouched.

@@ -195,7 +195,8 @@ __device__ __forceinline__ void line_tile_decode(int tile, int M, int li, int &m
 // NC = N at compile time (row offsets become immediates).
 // grid = min(ntiles, resident CTAs), block = NC threads (= 16 threads per chunk, P = NC / 16 even),
 // dynamic smem = 20 * NC * 16 (staging) + 2 * 2 * P * 16 * 16 (forward, backward exchange slots).
-// NB: neighbour-warp synchronisation (needs K <= 2) instead of CTA barriers; DIAG kernels use barriers.
+// NB: neighbour-warp synchronisation (needs K <= 2) instead of CTA barriers.  DIAG: also F, Fdot, mass partials, one per
+// (member, strip, warp): partials[((m * strips + strip) * (NC / 32) + warp) * 3].
 template <int NC, bool DIAG, bool NB>
 __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_y_line(const __grid_constant__ LineParams prm,
                                                                                    const double *__restrict__ C,
@@ -205,9 +206,7 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
     constexpr int LC = LINE_LC, NR = LC + 4, N = NC, NT = NC, P = NC / LC;
     constexpr size_t n2 = (size_t)N * N;
     extern __shared__ double2 sm2[];
-    __shared__ double red[16][3];
     __shared__ unsigned flagF[16], flagB[16];
-    static_assert(!(DIAG && NB), "the sampling kernels synchronise with CTA barriers");
     constexpr int NW = NC / 32;
     const int tid = threadIdx.x, li = tid & 15, c = tid >> 4, wid = tid >> 5;
     constexpr int strips = (NC + LINE_VALID - 1) / LINE_VALID;
@@ -306,16 +305,14 @@ __global__ void __launch_bounds__(NC, (NC <= 256 && !DIAG) ? 2 : 1) k_rhs_sweep_
         line_cp_async_commit();
 
         if (DIAG) {
-            // deterministic block sum: warp shuffle, then warps in fixed order
+            // deterministic sums without a CTA barrier (round 2): one partial per warp (fixed shuffle tree), k_finish adds
+            // the strips x warps partials of a member in index order; the sampling kernel can then use the same
+            // neighbour-warp synchronisation as the stepping kernel
             F = warp_sum(F); Fd = warp_sum(Fd); ms = warp_sum(ms);
-            if ((tid & 31) == 0) { red[tid >> 5][0] = F; red[tid >> 5][1] = Fd; red[tid >> 5][2] = ms; }
-            __syncthreads();
-            if (tid == 0) {
-                for (int q = 1; q < (NT >> 5); ++q) { F += red[q][0]; Fd += red[q][1]; ms += red[q][2]; }
-                double *o = partials + ((size_t)m * strips + strip) * 3;
+            if ((tid & 31) == 0) {
+                double *o = partials + (((size_t)m * strips + strip) * NW + wid) * 3;
                 o[0] = F; o[1] = Fd; o[2] = ms;
             }
-            __syncthreads();
             if (!prm.write) continue;         // diagnostics only (grid-uniform): no sweep
         }
 
