@@ -112,6 +112,16 @@ int ch_energy(ch_ctx *ctx, double *out, int on_device);
 /* Copy the current state out (stream-ordered; synchronises if the target is host memory). */
 int ch_get_state(ch_ctx *ctx, double *C, int on_device);
 
+/* The whole job from and to HOST memory: equivalent to ch_set_state(C_in, host) + ch_step(nsteps) + ch_get_state(C_out, host)
+ * (bitwise for the exact kernels; the series buffer registered with ch_set_series is filled the same way; afterwards the
+ * context holds the final state, n = nsteps, t0 = 0), but done member chunk by member chunk -- members are independent
+ * -- so that the host-to-device copy of chunk k + 1, the steps of chunk k and the device-to-host copy of
+ * chunk k - 1 overlap on three internal streams (ordered after everything already enqueued on the context's stream).
+ * `chunk` = members per chunk, 0 = library default (about 16 Mi grid points, at least 4 chunks).  C_in and C_out
+ * (ensemble * N^D doubles each, may be the same buffer) should be pinned host memory for the copies to be asynchronous.
+ * Synchronous: returns when everything has completed.  CUDA graphs are not used inside. */
+int ch_run_host(ch_ctx *ctx, const double *C_in, double *C_out, int nsteps, int chunk);
+
 /* Number of series samples written (enqueued) so far, steps taken since ch_set_state. */
 int ch_series_count(const ch_ctx *ctx);
 long long ch_step_count(const ch_ctx *ctx);

@@ -17,7 +17,7 @@ CH_OK, CH_EINVAL, CH_ENOMEM, CH_ECUDA, CH_ESTATE, CH_ENONFINITE = 0, -1, -2, -3,
 
 EXPORTS = [
     "ch_create", "ch_destroy", "ch_set_stream", "ch_workspace_bytes", "ch_attach_workspace",
-    "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_energy", "ch_get_state",
+    "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_run_host", "ch_energy", "ch_get_state",
     "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
     "ch_droplet_create", "ch_droplet_destroy", "ch_droplet_set_stream", "ch_droplet_set_state", "ch_droplet_get_state",
     "ch_droplet_integrate", "ch_droplet_replay", "ch_droplet_energy", "ch_droplet_last_error",
@@ -54,6 +54,7 @@ def lib():
         L.ch_set_time.argtypes = [vp, cd]
         L.ch_set_series.argtypes = [vp, dp, ci, ci]
         L.ch_step.argtypes = [vp, ci]
+        L.ch_run_host.argtypes = [vp, dp, dp, ci, ci]
         L.ch_energy.argtypes = [vp, dp, ci]
         L.ch_get_state.argtypes = [vp, dp, ci]
         L.ch_series_count.argtypes = [vp]
@@ -133,6 +134,14 @@ def ch_attach_workspace(ctx, tensor):
 def ch_set_state(ctx, C):
     p, dev = _ptr(C)
     _check(ctx, lib().ch_set_state(ctx, p, dev))
+
+
+def ch_run_host(ctx, C_in, C_out, nsteps, chunk=0):
+    """C_in, C_out: host arrays (numpy, or CPU torch tensors -- pinned for overlap) of the ensemble's shape."""
+    pi, di = _ptr(C_in)
+    po, do = _ptr(C_out)
+    assert di == 0 and do == 0, "ch_run_host takes host buffers"
+    _check(ctx, lib().ch_run_host(ctx, pi, po, nsteps, chunk))
 
 
 def ch_set_time(ctx, t0):

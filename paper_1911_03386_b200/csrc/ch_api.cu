@@ -86,6 +86,9 @@ struct ch_ctx {
     // one-pass local 2D step for small gamma dt (ch_local2d.cuh)
     bool local_ok;
     int loc_H, loc_resident;     // decay reach (ch_factor_reach), CTAs resident on the device
+    // ch_run_host: the kernels run on a member sub-range ("view"): M, total, C, w point at the view, these keep the whole
+    int Mfull, view_m0;
+    cudaStream_t rh_in, rh_comp, rh_out;     // its three internal streams (created on first use)
     long long launches;
     bool profiling;
     std::vector<ProfRec> prof;
@@ -249,6 +252,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
     if (!c) return fail(nullptr, CH_ENOMEM, "ch_create: out of host memory");
     c->M = ensemble; c->N = N; c->D = D; c->gamma = gamma; c->dt = dt;
     c->npts = ipow(N, D); c->total = c->npts * ensemble;
+    c->Mfull = ensemble; c->view_m0 = 0; c->rh_in = c->rh_comp = c->rh_out = nullptr;
     c->pow2 = (N & (N - 1)) == 0;
     c->LC = chunk_len_for(N);
     c->chunked = c->LC != 0;
@@ -437,6 +441,9 @@ extern "C" int ch_destroy(ch_ctx *ctx)
     if (ctx->dS2c) cudaFree(ctx->dS2c);
     if (ctx->gexec) cudaGraphExecDestroy(ctx->gexec);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+    if (ctx->rh_in) cudaStreamDestroy(ctx->rh_in);
+    if (ctx->rh_comp) cudaStreamDestroy(ctx->rh_comp);
+    if (ctx->rh_out) cudaStreamDestroy(ctx->rh_out);
     if (ctx->dS2_16) cudaFree(ctx->dS2_16);
     delete ctx;
     return CH_OK;
@@ -642,6 +649,9 @@ static void launch_rhs(ch_ctx *c, const double *C, double *r, double scale, bool
     else if (diag) launch_rhs_t<true, false>(c, C, r, scale);
     else launch_rhs_t<false, true>(c, C, r, scale);
 }
+
+// where the next sample of the members in view goes (ch_run_host steps member sub-ranges: view_m0, Mfull)
+static double *series_slot(const ch_ctx *c) { return c->series + ((size_t)c->cursor * c->Mfull + c->view_m0) * 4; }
 
 static void launch_finish(ch_ctx *c, double *out, double t, int nparts)
 {
@@ -988,7 +998,7 @@ static void launch_one_step(ch_ctx *ctx, bool sample)
     if (fuse_mode(ctx) == 5) {
         if (sample) {
             const int np_ = launch_diag_only(ctx);
-            launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt, np_);
+            launch_finish(ctx, series_slot(ctx), ctx->t0 + (double)ctx->n * ctx->dt, np_);
             ctx->cursor++; ctx->last_sampled = ctx->n;
         }
         launch_step_local(ctx);
@@ -997,7 +1007,7 @@ static void launch_one_step(ch_ctx *ctx, bool sample)
     if (fused) unscaled = launch_rhs_sweep_y(ctx, sample, true);
     else launch_rhs(ctx, ctx->C, ctx->w, ctx->rscale, sample, true);
     if (sample) {
-        launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt,
+        launch_finish(ctx, series_slot(ctx), ctx->t0 + (double)ctx->n * ctx->dt,
                       fused ? fused_parts(ctx) : rhs_parts_in_use(ctx));
         ctx->cursor++; ctx->last_sampled = ctx->n;
     }
@@ -1051,20 +1061,20 @@ static bool ensure_graph(ch_ctx *c)
     return true;
 }
 
-extern "C" int ch_step(ch_ctx *ctx, int nsteps)
+// samples a call of nsteps steps starting at step n0 will write: every n in [n0, n0 + nsteps] with n % stride == 0, not yet sampled
+static long long samples_ahead(const ch_ctx *ctx, int nsteps)
 {
-    if (!ctx) return CH_EINVAL;
-    if (nsteps < 0) return fail(ctx, CH_EINVAL, "ch_step: nsteps < 0");
-    if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_step: no state (call ch_set_state first)");
-    if (ctx->series) {
-        // samples this call will write: every n in [n0, n0 + nsteps] with n % stride == 0, not yet sampled
-        long long n0 = ctx->n, n1 = ctx->n + nsteps, cnt = 0;
-        long long first = ((n0 + ctx->stride - 1) / ctx->stride) * ctx->stride;
-        if (first <= n1) cnt = (n1 - first) / ctx->stride + 1;
-        if (first == ctx->last_sampled) cnt -= 1;
-        if (ctx->cursor + cnt > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_step: series full");
-    }
-    const bool graphs = graph_wanted(ctx);
+    if (!ctx->series) return 0;
+    long long n0 = ctx->n, n1 = ctx->n + nsteps, cnt = 0;
+    long long first = ((n0 + ctx->stride - 1) / ctx->stride) * ctx->stride;
+    if (first <= n1) cnt = (n1 - first) / ctx->stride + 1;
+    if (first == ctx->last_sampled) cnt -= 1;
+    return cnt;
+}
+
+// enqueue nsteps steps (and their samples) of the members in view on ctx->stream
+static void step_body(ch_ctx *ctx, int nsteps, bool graphs)
+{
     for (int s = 0; s < nsteps;) {
         const bool sample = ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n;
         if (!sample && graphs && ctx->dir3 == 0) {
@@ -1088,10 +1098,91 @@ extern "C" int ch_step(ch_ctx *ctx, int nsteps)
     }
     if (ctx->series && (ctx->n % ctx->stride == 0) && ctx->last_sampled != ctx->n) {
         const int np_ = launch_diag_only(ctx);
-        launch_finish(ctx, ctx->series + (size_t)ctx->cursor * ctx->M * 4, ctx->t0 + (double)ctx->n * ctx->dt, np_);
+        launch_finish(ctx, series_slot(ctx), ctx->t0 + (double)ctx->n * ctx->dt, np_);
         ctx->cursor++; ctx->last_sampled = ctx->n;
     }
+}
+
+extern "C" int ch_step(ch_ctx *ctx, int nsteps)
+{
+    if (!ctx) return CH_EINVAL;
+    if (nsteps < 0) return fail(ctx, CH_EINVAL, "ch_step: nsteps < 0");
+    if (!ctx->has_state) return fail(ctx, CH_ESTATE, "ch_step: no state (call ch_set_state first)");
+    if (ctx->cursor + samples_ahead(ctx, nsteps) > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_step: series full");
+    step_body(ctx, nsteps, graph_wanted(ctx));
     return check_launch(ctx, "ch_step");
+}
+
+// The whole job from and to HOST memory, member chunk by member chunk, with the H2D copy of chunk k + 1, the steps of chunk k
+// and the D2H copy of chunk k - 1 overlapping on three internal streams (members are independent: P:71).
+extern "C" int ch_run_host(ch_ctx *ctx, const double *C_in, double *C_out, int nsteps, int chunk)
+{
+    if (!ctx) return CH_EINVAL;
+    if (!C_in || !C_out) return fail(ctx, CH_EINVAL, "ch_run_host: C_in or C_out is NULL");
+    if (nsteps < 0 || chunk < 0) return fail(ctx, CH_EINVAL, "ch_run_host: nsteps < 0 or chunk < 0");
+    int rc = ensure_workspace(ctx);
+    if (rc) return rc;
+    if (!ctx->rh_in) {
+        CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->rh_in, cudaStreamNonBlocking));
+        CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->rh_comp, cudaStreamNonBlocking));
+        CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->rh_out, cudaStreamNonBlocking));
+    }
+    // as after ch_set_state: n = 0, t0 = 0, series cursor reset
+    ctx->has_state = true; ctx->n = 0; ctx->t0 = 0.0; ctx->cursor = 0; ctx->last_sampled = -1;
+    if (samples_ahead(ctx, nsteps) > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_run_host: series full");
+    const int M = ctx->M;
+    if (chunk == 0) {
+        // default: about 16 Mi points per chunk (copy and compute of a chunk take comparable time), at least 4 chunks
+        const size_t want = ((size_t)16 << 20) / ctx->npts;
+        chunk = (int)(want < 1 ? 1 : want);
+        if (chunk > (M + 3) / 4) chunk = (M + 3) / 4;
+        if (chunk < 1) chunk = 1;
+    }
+    if (chunk > M) chunk = M;
+    double *const Cfull = ctx->C, *const wfull = ctx->w;
+    const size_t total_full = ctx->total;
+    cudaStream_t user = ctx->stream;
+    cudaEvent_t ev_start = nullptr;
+    CUDA_TRY(ctx, cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+    cudaEventRecord(ev_start, user);                 // everything enqueued before this call comes first
+    cudaStreamWaitEvent(ctx->rh_in, ev_start, 0);
+    cudaStreamWaitEvent(ctx->rh_comp, ev_start, 0);
+    cudaStreamWaitEvent(ctx->rh_out, ev_start, 0);
+    const int dir0 = ctx->dir3;
+    long long n_end = 0; int cursor_end = 0; long long ls_end = -1;
+    double *Cend = Cfull, *wend = wfull;
+    cudaError_t err = cudaSuccess;
+    for (int m0 = 0; m0 < M && err == cudaSuccess; m0 += chunk) {
+        const int mc = m0 + chunk <= M ? chunk : M - m0;
+        const size_t off = (size_t)m0 * ctx->npts, cnt = (size_t)mc * ctx->npts;
+        cudaEvent_t ev_in = nullptr, ev_comp = nullptr;
+        err = cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming);
+        if (err == cudaSuccess) err = cudaEventCreateWithFlags(&ev_comp, cudaEventDisableTiming);
+        if (err != cudaSuccess) break;
+        err = cudaMemcpyAsync(Cfull + off, C_in + off, cnt * 8, cudaMemcpyHostToDevice, ctx->rh_in);
+        cudaEventRecord(ev_in, ctx->rh_in);
+        cudaStreamWaitEvent(ctx->rh_comp, ev_in, 0);
+        // the view: this chunk's members only
+        ctx->C = Cfull + off; ctx->w = wfull + off; ctx->M = mc; ctx->total = cnt; ctx->view_m0 = m0;
+        ctx->n = 0; ctx->cursor = 0; ctx->last_sampled = -1; ctx->dir3 = dir0; ctx->stream = ctx->rh_comp;
+        step_body(ctx, nsteps, false);
+        n_end = ctx->n; cursor_end = ctx->cursor; ls_end = ctx->last_sampled;
+        // the one-pass local step ping-pongs the two arrays: the final state of the view is where ctx->C points now
+        double *fin = ctx->C;
+        if (m0 == 0) { Cend = fin - off; wend = ctx->w - off; }
+        cudaEventRecord(ev_comp, ctx->rh_comp);
+        cudaStreamWaitEvent(ctx->rh_out, ev_comp, 0);
+        if (err == cudaSuccess) err = cudaMemcpyAsync(C_out + off, fin, cnt * 8, cudaMemcpyDeviceToHost, ctx->rh_out);
+        cudaEventDestroy(ev_in); cudaEventDestroy(ev_comp);
+    }
+    // back to the whole ensemble
+    ctx->C = Cend; ctx->w = wend; ctx->M = M; ctx->total = total_full; ctx->view_m0 = 0; ctx->stream = user;
+    ctx->n = n_end; ctx->cursor = cursor_end; ctx->last_sampled = ls_end;
+    cudaEventDestroy(ev_start);
+    cudaError_t e1 = cudaStreamSynchronize(ctx->rh_in), e2 = cudaStreamSynchronize(ctx->rh_comp), e3 = cudaStreamSynchronize(ctx->rh_out);
+    if (err == cudaSuccess) err = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+    if (err != cudaSuccess) return fail(ctx, CH_ECUDA, std::string("ch_run_host: ") + cudaGetErrorString(err));
+    return check_launch(ctx, "ch_run_host");
 }
 
 extern "C" int ch_energy(ch_ctx *ctx, double *out, int on_device)

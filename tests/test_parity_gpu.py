@@ -563,6 +563,43 @@ def test_flag_synchronised_kernels_repeat_bitwise_under_load(B, M, N, steps):
     e.close()
 
 
+@pytest.mark.parametrize("M,N,D,nsteps,stride,chunk,opts", [
+    (12, 256, 2, 37, 10, 5, None),            # uneven chunks (5, 5, 2), line kernel, sampling inside and at the end
+    (9, 512, 2, 20, 5, 0, None),              # default chunking
+    (5, 1024, 2, 7, 3, 2, None),              # cluster line kernel
+    (6, 64, 3, 12, 4, 4, None),               # 3D
+    (7, 320, 2, 15, 5, 3, None),              # one-pass local step (auto), odd number of steps: arrays end up swapped
+    (3, 24, 2, 9, 3, 1, None),                # generic path
+])
+def test_run_host_is_set_state_step_get_state(B, M, N, D, nsteps, stride, chunk, opts):
+    """ch_run_host (host -> chunk-pipelined H2D / steps / D2H on three streams -> host) against the plain
+    ch_set_state + ch_step + ch_get_state job: same final field, same series, same context state afterwards."""
+    import torch
+    C0 = inputs.initial_state(range(60, 60 + M), N, D, -0.2, 0.2)
+    ref, sref = run_gpu(B, C0, 1.0, 0.01, nsteps, stride, options=opts)
+    hin = torch.from_numpy(C0.copy()).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    e = B.Ensemble(M, N, D, 1.0, 0.01, options=opts)
+    local = D == 2 and B.ch_get_option(e.ctx, "fuse_mode") == 5
+    e.set_series(stride, nsteps // stride + 1)
+    B.ch_run_host(e.ctx, hin, hout, nsteps, chunk)
+    out, s = hout.numpy().copy(), e.series()
+    assert B.ch_step_count(e.ctx) == nsteps and B.ch_series_count(e.ctx) == nsteps // stride + 1
+    state_after = e.get_state()
+    # the context goes on from there like any other
+    e.set_series(stride, 8)
+    e.step(2 * stride)
+    cont = e.get_state()
+    e.close()
+    if local:                                   # chunking moves the CTA spans: equal to the truncation, not bitwise
+        assert np.abs(out - ref).max() <= 1e-15 and np.abs(s - sref).max() <= 1e-12 * np.abs(sref).max()
+    else:
+        assert np.array_equal(out, ref) and np.array_equal(s, sref)
+    assert np.array_equal(state_after, out)
+    ref2, _ = run_gpu(B, out, 1.0, 0.01, 2 * stride, stride, options=opts)
+    assert np.abs(cont - ref2).max() <= (1e-15 if local else 0.0)
+
+
 def test_equivariances_on_gpu(B):
     C0 = inputs.initial_state([3, 4], 128, 2, [0.0, -0.3], 0.2)
     base, _ = run_gpu(B, C0, 1.0, 0.01, 50, 50)
