@@ -189,7 +189,7 @@ static bool line_geometry(int N, int D, int *strips)
 
 static bool rhs3_stream_geometry(int N, int D, int *parts)
 {
-    if (D != 3 || (N != 64 && N != 128)) return false;
+    if (D != 3 || (N != 64 && N != 96 && N != 128)) return false;
     *parts = ((N + R3_VALID - 1) / R3_VALID) * (N / R3_ZR);
     return true;
 }
@@ -343,7 +343,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
             if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs3d_stream<NC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
             if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_rhs3d_stream<NC, false>, 4 * NC, smem); \
         }
-        X(64) X(128)
+        X(64) X(96) X(128)
 #undef X
         if (e == cudaSuccess) e = cudaGetDevice(&dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -629,6 +629,7 @@ static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
         const int grid = p.nunits < c->r3_resident ? p.nunits : c->r3_resident;
         const size_t smem = rhs3_stream_smem(c->N);
         if (c->N == 64) k_rhs3d_stream<64, DIAG><<<grid, 256, smem, c->stream>>>(p, C, r, c->partials);
+        else if (c->N == 96) k_rhs3d_stream<96, DIAG><<<grid, 384, smem, c->stream>>>(p, C, r, c->partials);
         else k_rhs3d_stream<128, DIAG><<<grid, 512, smem, c->stream>>>(p, C, r, c->partials);
         return;
     }

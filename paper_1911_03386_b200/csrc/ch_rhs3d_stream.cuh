@@ -1,4 +1,4 @@
-// ch_rhs3d_stream.cuh -- explicit RHS of the 3D step as a z-marching ("2.5-D") kernel, N in {64, 128}.
+// ch_rhs3d_stream.cuh -- explicit RHS of the 3D step as a z-marching ("2.5-D") kernel, N in {64, 96, 128}.
 // DESIGN.md section 5.
 //
 //   k_rhs3d_stream   r = scale * Lap_h mu(C),  mu = C^3 - C - gamma Lap_h C  (7-point Laplacians)    P:29-30, include/ch.h
@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(4 * NC, 1) k_rhs3d_stream(const __grid_constan
         const bool valid = li >= 1 && li < 15 && (X + 2 * (li - 1)) < N;
         const double *pC = C + (size_t)m * n3 + (size_t)(hw * RY) * N + gx;
         auto load_plane = [&](int zz, int slot) {
-            const double *p = pC + (size_t)((zz + N) & (N - 1)) * n2;
+            const double *p = pC + (size_t)((zz + N) % N) * n2;          // N is a compile-time constant
 #pragma unroll
             for (int j = 0; j < RY; ++j) line_cp_async16(stage + (slot * RY + j) * NT, p + j * N);
             line_cp_async_commit();

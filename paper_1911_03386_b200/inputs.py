@@ -61,6 +61,9 @@ CONFIGS = {
 # cases the one-pass local step serves.  Same recipe as cfg3 (asymmetric mixture, 2^25 points).
 CONFIGS["n768"] = dict(ensemble=57, N=768, D=2, gamma=1.0, dt=0.01, nsteps=20000, stride=50, cbar=-0.4, amp=0.05, seed0=5000)
 CONFIGS["n1000"] = dict(ensemble=32, N=1000, D=2, gamma=1.0, dt=0.01, nsteps=20000, stride=50, cbar=-0.4, amp=0.05, seed0=6000)
+# 3D shapes outside the streaming / plane-kernel sizes {64, 128} (they take the tile RHS + three separate sweeps, 72 B per update)
+CONFIGS["c96"] = dict(ensemble=38, N=96, D=3, gamma=1.0, dt=0.01, nsteps=10000, stride=50, cbar=-0.4, amp=0.05, seed0=7000)
+CONFIGS["c256"] = dict(ensemble=2, N=256, D=3, gamma=1.0, dt=0.01, nsteps=10000, stride=50, cbar=-0.4, amp=0.05, seed0=8000)
 
 
 def config_state(name: str, members=None) -> np.ndarray:

@@ -197,6 +197,25 @@ def test_3d_streaming_and_tile_rhs(B, oracle):
     assert_series_close(s[:, sub], so)
 
 
+def test_3d_streaming_rhs_at_96(B, oracle):
+    """96^3: not a power of two -- the z-marching RHS kernel (wrap by modulo) with the separate chunked sweeps, several
+    units per CTA, against the tile RHS kernel and the oracle (sampling every 10 steps: the DIAG variant too)."""
+    C0 = inputs.initial_state(range(3500, 3505), 96, 3, [0.0, -0.4, 0.2, -0.1, 0.3], 0.05)
+    e = B.Ensemble(5, 96, 3, 1.0, 0.01)
+    assert B.ch_get_option(e.ctx, "rhs3_stream") > 0 and B.ch_get_option(e.ctx, "sweep_xy") == 0
+    e.set_state(C0)
+    r, ro = e.rhs(), oracle.rhs(C0, 1.0, 0.01)
+    e.close()
+    assert np.abs(r - ro).max() <= 1e-13 * np.abs(ro).max()
+    C, s = run_gpu(B, C0, 1.0, 0.01, 40, 10)
+    Ct, st = run_gpu(B, C0, 1.0, 0.01, 40, 10, options={"rhs3": 1})
+    assert np.abs(C - Ct).max() <= 1e-13
+    assert_series_close(s, st, 1e-12)
+    Co, so = oracle.run(C0[[0, 4]], 1.0, 0.01, 40, 10)
+    assert np.abs(C[[0, 4]] - Co).max() <= FIELD_TOL
+    assert_series_close(s[:, [0, 4]], so)
+
+
 def test_3d_plane_sweep_paper_regime(B, oracle):
     """x + y sweeps of a z-plane in one kernel at gamma dt = 529 (long closures: shuffle scan in x, K-term sum in y),
     64^3 and 128^3, against the oracle."""
