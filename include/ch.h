@@ -137,8 +137,8 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *   "sweep"    0 auto, 1 force the generic thread-per-line sweeps, 2 force the chunked periodic-LU sweeps,
  *              3 parallel cyclic reduction for the x-axis of ch_sweep (N a power of two <= 4096)
  *   "fuse"     which 2D step runs: 0 auto, 1 three passes (RHS, x-sweep, y-sweep + update; 56 B per update),
- *              2 RHS fused into a cluster/st.async y-sweep, 3 the line kernel (N in {32, 64, 96, 128, 192, 256,
- *              384, 512}), 4 the cluster line kernel (N in {1024, 2048, 4096}); modes 2-4 finish with the
+ *              2 RHS fused into a cluster/st.async y-sweep, 3 the line kernel (N in {32, 64, 96, 128, 160, 192, 224,
+ *              256, 320, 384, 448, 512}), 4 the cluster line kernel (N in {1024, 2048, 4096}); modes 2-4 finish with the
  *              x-sweep fused with C += w (40 B per update); 5 the one-pass local step:
  *              RHS, y-sweep, x-sweep and update in one kernel that reads C^n once and writes C^{n+1} once (16 B per
  *              update), legal when the recurrences of the factorisation decay within 18 points to below 2^-56 of the

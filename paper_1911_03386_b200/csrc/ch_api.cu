@@ -174,7 +174,7 @@ static bool fused_geometry(int N, int D, int *CPB, int *CS, int *strips)
 
 // Line kernel geometry: whole lines of P = N / 16 chunks in one CTA of N threads; N is a template
 // parameter of the kernel, instantiated for the sizes below.
-#define LINE_SIZES(X) X(32) X(64) X(96) X(128) X(192) X(256) X(384) X(512)
+#define LINE_SIZES(X) X(32) X(64) X(96) X(128) X(160) X(192) X(224) X(256) X(320) X(384) X(448) X(512)
 static bool line_geometry(int N, int D, int *strips)
 {
     if (D != 2) return false;
@@ -582,7 +582,7 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         if (value == 5 && !ctx->local_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the one-pass local step needs D = 2, N % 4 == 0 and a decay reach <= 18 points (gamma dt <~ 0.012)");
         if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2 and N in {1024, 2048, 4096}");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
-        if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 192, 256, 384, 512}");
+        if (value == 3 && !ctx->line_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the line-fused step needs D = 2 and N in {32, 64, 96, 128, 160, 192, 224, 256, 320, 384, 448, 512}");
         ctx->opt_fuse = value;
         return CH_OK;
     }

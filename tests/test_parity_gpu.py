@@ -341,11 +341,11 @@ def test_generic_paths_end_to_end(B, oracle):
         assert_series_close(s, so)
 
 
-@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 128, 176, 192, 256, 352, 384, 512, 592, 1024])
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 128, 160, 176, 192, 224, 256, 320, 352, 384, 448, 512, 592, 1024])
 @pytest.mark.parametrize("gamma,dt", [(1.0, 0.01), (66.4, 7.97)])
 def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     """Every 2D step variant against the oracle: the line-fused step (RHS + y-sweep with whole lines
-    in one persistent CTA, N in {32, 64, 96, 128, 192, 256, 384, 512}; ragged last column strip, more tiles than
+    in one persistent CTA, N in {32, 64, 96, 128, 160, 192, 224, 256, 320, 384, 448, 512}; ragged last column strip, more tiles than
     resident CTAs at M = 40), the cluster-fused step (cluster sizes 1..8) and the three-pass step.
     N = 592 (37 chunks per line) has no legal split and must fall back to three passes by itself."""
     M = 2 if N <= 256 else 1
@@ -359,7 +359,7 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     e.close()
     assert (local != 0) == (gamma == 1.0 and N >= 64)          # one-pass local step: small gamma dt only
     assert (cs == 0) == (N == 592)
-    assert (line != 0) == (N in (32, 64, 96, 128, 192, 256, 384, 512))
+    assert (line != 0) == (N in (32, 64, 96, 128, 160, 192, 224, 256, 320, 384, 448, 512))
     assert (cline != 0) == (N == 1024)                         # flag kernel at K <= 2, scan kernel in the paper regime
     assert mode == (3 if line else (4 if cline else (5 if local else (2 if cs else 0))))
     variants = [{"fuse": 1}] + ([{"fuse": 5}] if local else []) + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
@@ -459,7 +459,7 @@ def test_local_step_is_selected_from_gamma_dt_with_a_host_bound(B):
             with pytest.raises(B.ChError):
                 B.ch_set_option(e.ctx, "fuse", 5)
         e.close()
-    for N, want in [(512, 3), (2048, 4), (768, 5), (1000, 5), (320, 5), (100, 5), (24, 0)]:
+    for N, want in [(512, 3), (320, 3), (2048, 4), (768, 5), (1000, 5), (352, 5), (100, 5), (24, 0)]:
         e = B.Ensemble(1, N, 2, 1.0, 0.01)
         assert B.ch_get_option(e.ctx, "fuse_mode") == want, N
         e.close()
@@ -505,7 +505,7 @@ def test_local_step_shapes(B, oracle, M, N, nsteps, gamma, dt):
         assert_series_close(s, sr, 1e-12)
 
 
-@pytest.mark.parametrize("M,N,steps", [(128, 512, 12), (9, 1000, 8), (3, 2048, 6), (74, 320, 16)])
+@pytest.mark.parametrize("M,N,steps", [(128, 512, 12), (9, 1000, 8), (3, 2048, 6), (74, 352, 16)])
 def test_local_step_is_deterministic(B, M, N, steps):
     """Warps of the one-pass kernel synchronise through per-warp mbarriers and three CTA barriers per block and drift
     apart in between: 20 repeats, half of them with a second stream keeping the GPU busy, must agree bitwise."""
@@ -587,7 +587,7 @@ def test_flag_synchronised_kernels_repeat_bitwise_under_load(B, M, N, steps):
     (9, 512, 2, 20, 5, 0, None),              # default chunking
     (5, 1024, 2, 7, 3, 2, None),              # cluster line kernel
     (6, 64, 3, 12, 4, 4, None),               # 3D
-    (7, 320, 2, 15, 5, 3, None),              # one-pass local step (auto), odd number of steps: arrays end up swapped
+    (7, 352, 2, 15, 5, 3, None),              # one-pass local step (auto), odd number of steps: arrays end up swapped
     (3, 24, 2, 9, 3, 1, None),                # generic path
 ])
 def test_run_host_is_set_state_step_get_state(B, M, N, D, nsteps, stride, chunk, opts):
