@@ -4,6 +4,7 @@
 #include <cmath>
 #include <complex>
 #include <cstring>
+#include <vector>
 
 namespace {
 
@@ -147,7 +148,7 @@ int ch_factor_reach(const ChFactor *f, double eps, int hmax)
 {
     // |h_k| summed far enough that the remainder is below 1e-40 of the total (rho < 1)
     const int KMAX = 4096;
-    static thread_local ld habs[KMAX];
+    std::vector<ld> habs(KMAX);
     ld h1 = 1, h2 = 0, G = 0;
     int n = 0;
     for (; n < KMAX; ++n) {
