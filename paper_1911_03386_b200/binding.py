@@ -25,7 +25,8 @@ EXPORTS = [
     "ch_kernel_kind_name", "ch_stats_moments", "ch_stats_hist", "ch_stats_fit", "ch_grid_doubling_error",
 ]
 
-_LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libch.so")
+# CH_LIBCH selects another build of the library (the debug build with in-kernel synchronisation assertions, build.py)
+_LIBPATH = os.environ.get("CH_LIBCH") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libch.so")
 _lib = None
 
 

@@ -41,5 +41,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+LIB_DEBUGSYNC = os.path.join(HERE, "libch_debugsync.so")
+
+
+def build_debug_sync(force: bool = False) -> str:
+    """libch_debugsync.so: the same library with -DCH_DEBUG_SYNC, i.e. with the in-kernel assertions on the sequence numbers
+    of the flag-synchronised kernels (ch_line2d.cuh).  Load it with CH_LIBCH=<path> (binding.py)."""
+    deps = sources() + glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh"))
+    if force or not os.path.exists(LIB_DEBUGSYNC) or any(os.path.getmtime(d) > os.path.getmtime(LIB_DEBUGSYNC) for d in deps):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        subprocess.run([nvcc] + NVCC_FLAGS + ["-DCH_DEBUG_SYNC", "-o", LIB_DEBUGSYNC] + sources(), check=True)
+    return LIB_DEBUGSYNC
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--debug-sync" in sys.argv:
+        print(build_debug_sync(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -44,6 +44,9 @@ __device__ __forceinline__ void cl_flag_wait(const unsigned *flag, unsigned seq)
     do {
         asm volatile("ld.acquire.cluster.shared::cta.u32 %0, [%1];\n" : "=r"(v) : "r"(a) : "memory");
     } while (v < seq);
+#ifdef CH_DEBUG_SYNC
+    if (v != seq) __trap();           // the neighbouring CTA is never a whole tile ahead (ch_line2d.cuh, flag_wait)
+#endif
 }
 __device__ __forceinline__ void cl_sync_all()
 {

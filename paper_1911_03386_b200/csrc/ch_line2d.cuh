@@ -70,8 +70,20 @@ __device__ __forceinline__ double hshfl_down(double v) { return __shfl_down_sync
 // the warp itself and ONE neighbouring warp.  Instead of a CTA-wide barrier each warp publishes a
 // sequence number (release) after writing its exchange slots and polls its neighbour's (acquire), so
 // the warps of a CTA drift apart and their load / fp64 / store phases overlap.
+// CH_DEBUG_SYNC (python -m paper_1911_03386_b200.build --debug-sync -> libch_debugsync.so; tests/test_parity_gpu.py runs the
+// stress shapes against it): the protocol's invariants are checked in the kernel and a violation traps.  A warp publishes
+// tile numbers in steps of exactly one, and when a waiter's condition becomes true the flag it polls equals the tile it
+// waits for -- a neighbour can never be a whole tile ahead, because it rewrites a slot only after the reader of that slot
+// has published the NEXT flag of the tile in between.
 __device__ __forceinline__ void flag_release(unsigned *flag, unsigned seq)
 {
+#ifdef CH_DEBUG_SYNC
+    {
+        unsigned old;
+        asm volatile("ld.relaxed.cta.shared.u32 %0, [%1];\n" : "=r"(old) : "r"((unsigned)__cvta_generic_to_shared(flag)) : "memory");
+        if (old + 1u != seq) __trap();
+    }
+#endif
     asm volatile("st.release.cta.shared.u32 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(flag)), "r"(seq) : "memory");
 }
 __device__ __forceinline__ void flag_wait(const unsigned *flag, unsigned seq)
@@ -81,6 +93,9 @@ __device__ __forceinline__ void flag_wait(const unsigned *flag, unsigned seq)
     do {
         asm volatile("ld.acquire.cta.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(a) : "memory");
     } while (v < seq);
+#ifdef CH_DEBUG_SYNC
+    if (v != seq) __trap();
+#endif
 }
 
 // keeps the compiler from carrying values derived from x across the long tile body in registers:

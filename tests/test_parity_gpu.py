@@ -619,6 +619,41 @@ def test_run_host_is_set_state_step_get_state(B, M, N, D, nsteps, stride, chunk,
     assert np.abs(cont - ref2).max() <= (1e-15 if local else 0.0)
 
 
+def test_flag_protocol_invariants_in_the_debug_build(B, tmp_path):
+    """libch_debugsync.so (-DCH_DEBUG_SYNC) checks inside the kernels that every warp publishes tile numbers in steps of
+    exactly one and that a waiter never finds its neighbour a whole tile ahead (ch_line2d.cuh, ch_cline2d.cuh); a violation
+    traps.  The stress shapes run against it in a separate process (the library path is fixed at import) and must finish
+    and reproduce the production library's fields bitwise."""
+    import os
+    import subprocess
+    import sys
+    from paper_1911_03386_b200 import build
+    lib = build.build_debug_sync()
+    shapes = [(9, 512, 12), (17, 512, 8), (33, 256, 10), (5, 1024, 6), (3, 2048, 5), (1, 4096, 4)]
+    refs = {}
+    for M, N, steps in shapes:
+        C0 = inputs.initial_state(range(700, 700 + M), N, 2, -0.3, 0.1)
+        refs[(M, N)], _ = run_gpu(B, C0, 1.0, 0.01, steps, 2)
+        np.save(tmp_path / f"ref_{M}_{N}.npy", refs[(M, N)])
+    script = f"""
+import sys, numpy as np
+sys.path.insert(0, {str(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))!r})
+from paper_1911_03386_b200 import binding as B, inputs
+assert B._LIBPATH.endswith("libch_debugsync.so")
+for M, N, steps in {shapes!r}:
+    C0 = inputs.initial_state(range(700, 700 + M), N, 2, -0.3, 0.1)
+    for rep in range(3):
+        e = B.Ensemble(M, N, 2, 1.0, 0.01)
+        assert B.ch_get_option(e.ctx, "fuse_mode") in (3, 4)
+        e.set_state(C0); e.set_series(2, steps // 2 + 1); e.step(steps)
+        C = e.get_state(); e.close()
+        assert np.array_equal(C, np.load({str(tmp_path)!r} + f"/ref_{{M}}_{{N}}.npy")), (M, N, rep)
+print("debug build ok")
+"""
+    r = subprocess.run([sys.executable, "-c", script], env={**os.environ, "CH_LIBCH": lib}, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "debug build ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
 def test_equivariances_on_gpu(B):
     C0 = inputs.initial_state([3, 4], 128, 2, [0.0, -0.3], 0.2)
     base, _ = run_gpu(B, C0, 1.0, 0.01, 50, 50)
