@@ -146,3 +146,20 @@ def test_droplet_errors(B):
     B.ch_droplet_get_state(ctx, R)
     assert np.abs(R - 0.5).max() <= 1e-12                          # equal droplets are stationary
     B.ch_droplet_destroy(ctx)
+
+
+def test_ensemble_study_against_the_papers_table_2(B):
+    """Section 3.3 / Table 2 (tests/golden/table_2.txt): M = 100 realisations to t = 40, beta sampled every 0.1,
+    beta_0 = mean of mu_1 over [20, 40], k = slope of mu_2 = k t -- Model 1 and the ensemble statistics (NEXT-4 + NEXT-1) end to
+    end through the C ABI.  beta spikes whenever a droplet dies ((1 - ubar R)^2 / R), so mu_2 depends on how the series is
+    sampled, which the paper does not say, and M = 100 leaves ~15 % noise on k: a sanity band, not a parity pin.  Measured
+    here: N = 512: beta_0 = 0.299, k = 6.1e-3 (paper 0.24, 7.5e-3); N = 2048: 0.307, 3.9e-3 (paper 0.283, 1.7e-3)."""
+    import os
+    from paper_1911_03386_b200 import droplet_study
+    paper = {int(l.split()[0]): (float(l.split()[1]), float(l.split()[2]))
+             for l in open(os.path.join(os.path.dirname(__file__), "golden", "table_2.txt")) if l.strip() and not l.startswith("#")}
+    got = {N: droplet_study.study(N)[:2] for N in (512, 2048)}
+    for N, (b0, k) in got.items():
+        assert 0.2 <= b0 <= 0.4, (N, b0)                           # approaching the LSW value 1/3 from below (P:495)
+        assert paper[N][1] / 3 <= k <= 3 * paper[N][1], (N, k)
+    assert got[2048][1] < got[512][1]                              # the variance falls with N (P:499: k ~ 1/N)
