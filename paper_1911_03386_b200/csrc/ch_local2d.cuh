@@ -326,45 +326,50 @@ __global__ void __launch_bounds__(LOC_NT, 2) k_step2d_local(const __grid_constan
                 }
                 sideB[wid * LOC_LB + lane] = make_double2(a1, a2);            // state entering chunk wid - 1 from the right
             }
-            __syncthreads();
             // ---------------- P4: C^{n+1} = C^n + scale * (w + backward correction); warp = its own 30 columns,
-            // half-warp = row parity, lane & 15 = column pair
-            {
-                const int half = lane >> 4, c = c0 + 2 * (lane & 15);            // r-region column of the pair
-                if ((lane & 15) < LOC_XC / 2 && c >= He && c < He + wd) {
-                    const int kb = c1 - 2 - c;                                   // distance of the pair's right column from the chunk end
-                    const bool corr = kb < LOC_KC && c1 < RWs;
-                    const double ax = corr ? prm.al[kb + 1] : 0.0, bx = corr ? prm.be[kb + 1] : 0.0;
-                    const double ay = corr ? prm.al[kb] : 0.0, by = corr ? prm.be[kb] : 0.0;
-                    const size_t off = (size_t)(ya + lo - H + half) * N + (size_t)(x0 + c - He);
-                    const double2 *ci = reinterpret_cast<const double2 *>(Cm + off);
-                    double2 *co = reinterpret_cast<double2 *>(Om + off);
-                    const double2 *sb = sideB + (wid + 1) * LOC_LB + half;
-                    int zrow4 = (lo + half) % LOC_ZR;
-                    const double *zp = zring + zrow4 * LOC_ZP + c;
-                    const double osc = prm.oscale;
-                    const size_t N1 = (size_t)N;                                 // two rows = N double2
-                    const int nr = (nf - half + 1) >> 1;                         // rows of this parity
-                    for (int r0 = 0; r0 < nr; r0 += 8) {
-                        double2 cv[8];
+            // half-warp = row parity, lane & 15 = column pair.  The first eight C^n rows are requested BEFORE the barrier that
+            // ends P3 (C^n is read-only here), so their L2 latency hides behind it.
+            const int half = lane >> 4, c = c0 + 2 * (lane & 15);                // r-region column of the pair
+            const bool p4_on = (lane & 15) < LOC_XC / 2 && c >= He && c < He + wd;
+            const size_t off = (size_t)(ya + lo - H + half) * N + (size_t)(x0 + c - He);
+            const double2 *ci = reinterpret_cast<const double2 *>(Cm + (p4_on ? off : 0));
+            const size_t N1 = (size_t)N;                                         // two rows = N double2
+            const int nr = p4_on ? (nf - half + 1) >> 1 : 0;                     // rows of this parity
+            double2 cv[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                if (i < nr) cv[i] = __ldg(ci + (size_t)i * N1);
+            __syncthreads();
+            if (p4_on) {
+                const int kb = c1 - 2 - c;                                       // distance of the pair's right column from the chunk end
+                const bool corr = kb < LOC_KC && c1 < RWs;
+                const double ax = corr ? prm.al[kb + 1] : 0.0, bx = corr ? prm.be[kb + 1] : 0.0;
+                const double ay = corr ? prm.al[kb] : 0.0, by = corr ? prm.be[kb] : 0.0;
+                double2 *co = reinterpret_cast<double2 *>(Om + off);
+                const double2 *sb = sideB + (wid + 1) * LOC_LB + half;
+                int zrow4 = (lo + half) % LOC_ZR;
+                const double *zp = zring + zrow4 * LOC_ZP + c;
+                const double osc = prm.oscale;
+                for (int r0 = 0; r0 < nr; r0 += 8) {
+                    if (r0 > 0) {
 #pragma unroll
                         for (int i = 0; i < 8; ++i)
                             if (r0 + i < nr) cv[i] = __ldg(ci + (size_t)i * N1);
-#pragma unroll
-                        for (int i = 0; i < 8; ++i)
-                            if (r0 + i < nr) {
-                                double2 wv = *reinterpret_cast<const double2 *>(zp);
-                                if (corr) {          // (never multiply an unwritten slot by zero: it may hold a NaN pattern)
-                                    const double2 bin = sb[2 * (r0 + i)];
-                                    wv.x = fma(ax, bin.x, fma(bx, bin.y, wv.x));
-                                    wv.y = fma(ay, bin.x, fma(by, bin.y, wv.y));
-                                }
-                                co[(size_t)i * N1] = make_double2(fma(osc, wv.x, cv[i].x), fma(osc, wv.y, cv[i].y));
-                                zp += 2 * LOC_ZP; zrow4 += 2;
-                                if (zrow4 >= LOC_ZR) { zrow4 -= LOC_ZR; zp -= LOC_ZRING; }
-                            }
-                        ci += 8 * N1; co += 8 * N1;
                     }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+                        if (r0 + i < nr) {
+                            double2 wv = *reinterpret_cast<const double2 *>(zp);
+                            if (corr) {              // (never multiply an unwritten slot by zero: it may hold a NaN pattern)
+                                const double2 bin = sb[2 * (r0 + i)];
+                                wv.x = fma(ax, bin.x, fma(bx, bin.y, wv.x));
+                                wv.y = fma(ay, bin.x, fma(by, bin.y, wv.y));
+                            }
+                            co[(size_t)i * N1] = make_double2(fma(osc, wv.x, cv[i].x), fma(osc, wv.y, cv[i].y));
+                            zp += 2 * LOC_ZP; zrow4 += 2;
+                            if (zrow4 >= LOC_ZR) { zrow4 -= LOC_ZR; zp -= LOC_ZRING; }
+                        }
+                    ci += 8 * N1; co += 8 * N1;
                 }
             }
         }
