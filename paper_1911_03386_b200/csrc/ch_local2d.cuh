@@ -16,7 +16,8 @@
 // Per block of 32 rows:
 //   P1 (warp w, lane l = r-region column 30 w + l - 1; lanes 1..30 produce, warps overlap by two columns)
 //        the warp stages the 34 C columns it needs itself: one cp.async.bulk per row issued by an elected lane, completion on
-//        the warp's own three mbarriers, 12-row ring, L2 prefetch LOC_PF rows ahead.  Rolling register window: mu of the
+//        the warp's own three mbarriers, 12-row ring (an extra L2 prefetch ahead of it measured SLOWER: 0.2585 vs
+//        0.2521 ms on CFG3, and read 9 % more DRAM bytes).  Rolling register window: mu of the
 //        next row (x-neighbours of C from the ring, of mu by shuffle), r = Lap_h mu, forward y-recurrence z (exact
 //        streaming, state in registers), z -> z-ring.  No CTA barrier: warps drift apart, load / fp64 phases overlap.
 //   P2 (same thread, its own column)   backward y-recurrence from a zero state at the newest row, H throw-away rows, in
@@ -46,7 +47,6 @@
 #define LOC_WC 34                         // C columns a warp stages: its 32 + one on either side
 #define LOC_SR 12                         // rows of a warp's C staging ring: 3 groups of 4
 #define LOC_KC LOC_HMAX                   // points of a chunk the state of its neighbour still reaches
-#define LOC_PF 24                         // rows the L2 prefetch runs ahead of the staging fetches
 
 struct LocalParams {
     double np, nq;                  // recurrence  z_i = b_i + np z_{i-1} + nq z_{i-2}
@@ -165,14 +165,8 @@ __global__ void __launch_bounds__(LOC_NT, 2) k_step2d_local(const __grid_constan
         const double *lsrc = Cm + (size_t)lgy * N + gxw;
         unsigned ldst = cws, lbar = mb;
         int lu = 0;                                  // next C row to fetch
-        // L2 prefetch runs LOC_PF rows ahead of the fetches: lanes 0..11 = (row of the group, 128-byte line of its 272 bytes)
-        int pgy = (lgy + LOC_PF + (lane >> 2)) % N;
-        const char *psrc = reinterpret_cast<const char *>(Cm + (size_t)pgy * N + gxw) + (lane & 3) * 128;
         auto issue_group = [&]() {                   // the next 4 C rows into ring rows lu % 12 ..
             if (lu < NU) {                           // NU is a multiple of 4: a group is fetched whole or not at all
-                if (lane < 12 && (lane & 3) < 3) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(psrc));
-                pgy += 4; psrc += (size_t)4 * N * 8;
-                if (pgy >= N) { pgy -= N; psrc -= n2 * 8; }
                 if (loc_elect_one()) {
                     loc_mbar_expect_tx(lbar, 4 * ROWB);
                     if (lgy + 4 <= N && wa == LOC_WC) {          // the common case: no periodic wrap inside the group
