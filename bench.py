@@ -43,7 +43,7 @@ ALGO_BYTES = {
 NCU_TRAFFIC_BYTES = {
     ("cfg3", "sweep_x_update"): (749.5e6, "profiles/r01_v8_ncu_full_cfg3.md"),
     ("cfg3", "rhs_sweep_y"): (485.6e6, "profiles/r01_v8_ncu_full_cfg3.md"),
-    ("cfg3", "step_local"): (695.6e6, "profiles/r02_ncu_full_local.md"),
+    ("cfg3", "step_local"): (656.1e6, "profiles/r02_ncu_full_local.md"),
 }
 
 
