@@ -831,7 +831,7 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
     p.M = c->M;
     {   // stepping kernels pack the ragged leftover strips of two members into one tile (ch_line2d.cuh, LineTiling)
         const int SF = c->N / LINE_VALID, REM = c->N - SF * LINE_VALID;
-        if (!diag && REM > 0 && REM <= 12) p.ntiles = (c->M / 2) * (2 * SF + 1) + (c->M & 1) * (SF + 1);
+        if (!diag && REM > 0 && REM <= 12) p.ntiles = line_packed_tiles(c->N, c->M);
     }
     const int grid = p.ntiles < c->l_resident ? p.ntiles : c->l_resident;
     const size_t smem = line_smem(c->N);

@@ -164,43 +164,51 @@ __device__ __forceinline__ void line_scan_closure(const LineParams &prm, double2
 }
 
 // Tiling of the columns.  Plain: ceil(NC / 28) strips per member, the last one ragged.  Packed (stepping kernels,
-// when the NC % 28 leftover columns fit half a half-warp): the leftover strips of members 2j and 2j+1 share ONE
-// tile -- lanes 0..7 work on member 2j, lanes 8..15 on member 2j+1 -- so a ragged strip costs half a tile
-// (N = 512, 128 members: 2432 -> 2368 tiles = exactly 16 rounds of 148 CTAs).
+// when the NC % 28 leftover columns fit a fraction of a half-warp): the leftover strips of G consecutive members share
+// ONE tile -- G = 2: lanes 0..7 work on member 2j, lanes 8..15 on member 2j+1 (leftover <= 12 columns); G = 4: four
+// lanes per member (leftover <= 4 columns) -- so a ragged strip costs 1/G of a tile
+// (N = 512, 128 members: 2432 -> 2368 tiles = exactly 16 rounds of 148 CTAs; N = 256, 64 members: 640 -> 592 tiles =
+// exactly 2 rounds of 2 x 148 CTAs).
 template <int NC>
 struct LineTiling {
     static constexpr int SF = NC / LINE_VALID, REM = NC - SF * LINE_VALID;
     static constexpr bool PACKABLE = REM > 0 && REM <= 12;
+    static constexpr int G = REM <= 4 ? 4 : 2;          // members per shared leftover tile
 };
+static inline int line_packed_tiles(int N, int M)
+{
+    const int SF = N / LINE_VALID, REM = N - SF * LINE_VALID, G = REM <= 4 ? 4 : 2;
+    return (M / G) * (G * SF + 1) + ((M % G) ? (M % G) * SF + 1 : 0);
+}
 
 // member, first column (wrapped, even) and "produces output" of half-warp lane li in `tile`.
-// Packed order: members come in pairs; pair p owns the PT = 2 SF + 1 consecutive tiles p PT .. (p + 1) PT - 1:
-// SF full strips of member 2p, SF of member 2p + 1, then the tile their leftover strips share (so a member's
-// tiles are complete PT tiles after its pair started: the one-kernel step of ch_step2d relies on it).  An odd
-// ensemble ends with a lone member: SF full strips and a half-idle leftover tile.
+// Packed order: members come in groups of G; group p owns the PT = G SF + 1 consecutive tiles p PT .. (p + 1) PT - 1:
+// SF full strips of each of its members in turn, then the tile their leftover strips share.  An ensemble that is not
+// a multiple of G ends with a short group: SF full strips per member and a partly idle leftover tile.
 template <int NC, bool PACK>
 __device__ __forceinline__ void line_tile_decode(int tile, int M, int li, int &m, int &gx, bool &ok)
 {
     constexpr int strips = (NC + LINE_VALID - 1) / LINE_VALID, SF = LineTiling<NC>::SF, REM = LineTiling<NC>::REM;
-    constexpr int PT = 2 * SF + 1;
+    constexpr int G = LineTiling<NC>::G, S = 16 / G, PT = G * SF + 1;
     if (!PACK) {
         const int strip = tile % strips;
         m = tile / strips;
         gx = strip * LINE_VALID - 2 + 2 * li;
         ok = li >= 1 && li < 15 && gx < NC;
     } else {
-        const int pair = tile / PT, k = tile - pair * PT;
-        const bool lone = 2 * pair + 1 >= M;                 // last member of an odd ensemble
-        if (k < SF || (!lone && k < 2 * SF)) {
-            m = 2 * pair + (k >= SF);
-            gx = (k >= SF ? k - SF : k) * LINE_VALID - 2 + 2 * li;
+        const int grp = tile / PT, k = tile - grp * PT;
+        const int nm = (M - G * grp) < G ? (M - G * grp) : G;      // members of this group
+        if (k < nm * SF) {
+            const int q = k / SF;
+            m = G * grp + q;
+            gx = (k - q * SF) * LINE_VALID - 2 + 2 * li;
             ok = li >= 1 && li < 15;
         } else {
-            const int l8 = li & 7;
-            m = 2 * pair + (li >> 3);
-            gx = SF * LINE_VALID - 2 + 2 * l8;
-            ok = l8 >= 1 && l8 <= REM / 2 && m < M;
-            if (m >= M) m = M - 1;              // the idle half works on valid memory and stores nothing
+            const int ls = li & (S - 1);
+            m = G * grp + li / S;
+            gx = SF * LINE_VALID - 2 + 2 * ls;
+            ok = ls >= 1 && ls <= REM / 2 && m < M;
+            if (m >= M) m = M - 1;              // the idle lanes work on valid memory and store nothing
         }
     }
     if (gx < 0) gx += NC;

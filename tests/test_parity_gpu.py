@@ -370,10 +370,12 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
         assert_series_close(s, so, rtol)
 
 
-@pytest.mark.parametrize("M,N", [(1, 512), (3, 512), (5, 256), (2, 96), (7, 64), (1, 32)])
+@pytest.mark.parametrize("M,N", [(1, 512), (3, 512), (5, 256), (6, 256), (7, 256), (8, 256), (2, 96), (7, 64), (1, 32), (4, 32),
+                                 (6, 32), (11, 32)])
 def test_line_kernel_packed_leftover_strips(B, oracle, M, N):
-    """Stepping kernels pack the NC % 28 leftover columns of two members into one tile (lanes 0-7 / 8-15 of the
-    half-warps); odd ensembles leave the second half of the last packed tile idle.  Against the oracle."""
+    """Stepping kernels pack the NC % 28 leftover columns of two members (lanes 0-7 / 8-15 of the half-warps), or of
+    four members when they are <= 4 columns (N = 256, 32: four lanes each), into one tile; ensembles that are not a
+    multiple of the group leave part of the last packed tile idle.  Against the oracle."""
     C0 = inputs.initial_state(range(600, 600 + M), N, 2, -0.25, 0.1)
     nsteps = 30 if N >= 256 else 100
     C, s = run_gpu(B, C0, 1.0, 0.01, nsteps, 10, options={"fuse": 3})
