@@ -109,6 +109,26 @@ int ch_step(ch_ctx *ctx, int nsteps);
  * call synchronises the stream and returns CH_ENONFINITE if any F is not finite. */
 int ch_energy(ch_ctx *ctx, double *out, int on_device);
 
+/* The same {F, dF/dt, beta, mass} (eq. (4), eq. (6); readings G3-G6) WITHOUT A CONTEXT AND WITHOUT ANY
+ * ALLOCATION -- for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it).  C_dev: DEVICE field [ensemble][N^D] (layout as ch_set_state), out_dev: DEVICE double[ensemble][4],
+ * t: the time beta is taken at (beta = -t dF/dt / F, 0 if F == 0); h = 1; enqueued on cuda_stream (a cudaStream_t, NULL =
+ * the legacy default stream), nothing synchronises; the CUDA device that is current must own both buffers.  The reduction
+ * partials live in a file-scope __device__ array of CH_ENERGY_STATIC_MAX_PARTS x 3 doubles (1.5 MiB, held by every GPU
+ * that loads the library until the process exits); a call needs ensemble * ceil(N^D / CH_ENERGY_STATIC_PART_POINTS) of
+ * them and is REJECTED with CH_EINVAL (nothing enqueued) beyond that, e.g. above 1024 members of 512^2, 64 of 2048^2 or 128 of
+ * 128^3 (2 GiB of state): use ch_energy, or split the ensemble over several calls.  The array is shared by every call and keeps the
+ * last call's contents (nothing in it has to start at zero: a call writes every slot it reads), so CALLS THAT OVERLAP ON
+ * THE GPU -- different streams without ordering, or different host threads -- RACE; calls ordered on one stream do not.
+ * The first call on a device looks the array's device address up (cudaGetSymbolAddress; make that call outside graph
+ * capture).  Calls no cudaMalloc, cudaFree or allocating library routine.  Slower than ch_energy (no shared-memory
+ * tiles); same values to round-off.  Errors: CH_EINVAL (NULL pointer, ensemble < 1, N < 8, D not in {2, 3}, gamma <= 0,
+ * too large), CH_ECUDA; the message goes to errbuf (may be NULL) as a NUL-terminated string of at most errlen bytes. */
+#define CH_ENERGY_STATIC_PART_POINTS 4096
+#define CH_ENERGY_STATIC_MAX_PARTS 65536
+int ch_energy_static(const double *C_dev, int ensemble, int N, int D, double gamma, double t, double *out_dev,
+                     void *cuda_stream, char *errbuf, size_t errlen);
+
 /* Copy the current state out (stream-ordered; synchronises if the target is host memory). */
 int ch_get_state(ch_ctx *ctx, double *C, int on_device);
 

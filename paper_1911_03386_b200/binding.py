@@ -17,7 +17,7 @@ CH_OK, CH_EINVAL, CH_ENOMEM, CH_ECUDA, CH_ESTATE, CH_ENONFINITE = 0, -1, -2, -3,
 
 EXPORTS = [
     "ch_create", "ch_destroy", "ch_set_stream", "ch_workspace_bytes", "ch_attach_workspace",
-    "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_run_host", "ch_energy", "ch_get_state",
+    "ch_set_state", "ch_set_time", "ch_set_series", "ch_step", "ch_run_host", "ch_energy", "ch_energy_static", "ch_get_state",
     "ch_series_count", "ch_step_count", "ch_rhs", "ch_sweep", "ch_set_option", "ch_get_option",
     "ch_droplet_create", "ch_droplet_destroy", "ch_droplet_set_stream", "ch_droplet_set_state", "ch_droplet_get_state",
     "ch_droplet_integrate", "ch_droplet_replay", "ch_droplet_energy", "ch_droplet_last_error",
@@ -57,6 +57,7 @@ def lib():
         L.ch_step.argtypes = [vp, ci]
         L.ch_run_host.argtypes = [vp, dp, dp, ci, ci]
         L.ch_energy.argtypes = [vp, dp, ci]
+        L.ch_energy_static.argtypes = [dp, ci, ci, ci, cd, cd, dp, vp, ctypes.c_char_p, ctypes.c_size_t]
         L.ch_get_state.argtypes = [vp, dp, ci]
         L.ch_series_count.argtypes = [vp]
         L.ch_step_count.argtypes = [vp]
@@ -160,6 +161,16 @@ def ch_step(ctx, nsteps):
 def ch_energy(ctx, out):
     p, dev = _ptr(out)
     _check(ctx, lib().ch_energy(ctx, p, dev))
+
+
+def ch_energy_static(C, gamma, t, out, stream=None):
+    """C: CUDA tensor [ensemble][N]^D, out: CUDA tensor [ensemble][4] (output).  No context, no allocation (include/ch.h)."""
+    M, N, D = C.shape[0], C.shape[1], C.dim() - 1
+    assert C.is_cuda and out.is_cuda and C.is_contiguous() and out.is_contiguous() and tuple(out.shape) == (M, 4)
+    err = ctypes.create_string_buffer(512)
+    rc = lib().ch_energy_static(C.data_ptr(), M, N, D, gamma, t, out.data_ptr(), ctypes.c_void_p(stream or 0), err, 512)
+    if rc != CH_OK:
+        raise ChError(rc, err.value.decode())
 
 
 def ch_get_state(ctx, C):
