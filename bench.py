@@ -40,6 +40,10 @@ ALGO_BYTES = {
 # value = (bytes per launch, the committed capture it was read from).  One launch under `ncu --set full`: caches are
 # flushed before the launch, so the L2 hits the live step gets from walking the ensemble up in one kernel and down in
 # the next do not show, and part of the write-back is still in L2 when the launch ends.
+# member-resident stepping: DFMA + DADD + DMUL per grid-point update (ncu, profiles/r02_ncu_full_resident.md) and the fp64 peak
+RESIDENT_FP64_INSTR_PER_UPDATE = 29.65
+ALU_PEAK_TINSTR = 148 * 64 * 1.965e9 / 1e12
+
 NCU_TRAFFIC_BYTES = {
     ("cfg3", "sweep_x_update"): (749.5e6, "profiles/r01_v8_ncu_full_cfg3.md"),
     ("cfg3", "rhs_sweep_y"): (485.6e6, "profiles/r01_v8_ncu_full_cfg3.md"),
@@ -249,28 +253,48 @@ def run_ours(args):
             gbs = pts * ALGO_BYTES[D][kind] / (avg * 1e-3) / 1e9
             kernels[kind] = {"launches": cnt, "avg_ms": avg, "algo_bytes_per_update": ALGO_BYTES[D][kind],
                              "achieved_gbs": gbs, "frac": gbs / peak}
+    if prof.get("step_resident", (0.0, 0))[1]:
+        # member-resident stepping (fuse_mode 6): ONE launch runs all K steps out of shared memory, so the bound is the fp64
+        # pipe, not HBM: fp64 instructions per update counted by ncu, peak from the unit count and clock
+        ms, cnt = prof["step_resident"]
+        tinstr = pts * K * RESIDENT_FP64_INSTR_PER_UPDATE / (ms * 1e-3) / 1e12
+        kernels["step_resident"] = {"launches": cnt, "avg_ms": ms / cnt, "steps_per_launch": K,
+                                    "fp64_instr_per_update": RESIDENT_FP64_INSTR_PER_UPDATE, "achieved_tinstr_s": tinstr,
+                                    "frac": tinstr / ALU_PEAK_TINSTR, "hbm_bytes_per_update": 16.0 / K}
     total_kernel_ms = sum(ms for ms, _ in prof.values())
     # bytes one step must move in the pass structure that ran: fused 2D step 16 + 24 = 40 B per update
     # (DESIGN.md section 5), three-pass 2D 56 B, four-pass 3D 72 B
     fused = "sweep_x_update" in kernels
     step_bytes = 16 if "step_local" in kernels else (40 if fused else (56 if D == 2 else (56 if "sweep_xy" in kernels else 72)))
     model_bytes = 56 if D == 2 else 72
-    main_kinds = {k: v for k, v in kernels.items() if not k.endswith("_diag")} or kernels
-    dom = max(main_kinds, key=lambda k: main_kinds[k]["avg_ms"] * main_kinds[k]["launches"])
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES.get((name, dom), (None, None))[0],
-                "traffic_source": NCU_TRAFFIC_BYTES.get((name, dom), (None, None))[1],
-                "peak_source": peak_src, "share_of_step": kernels[dom]["avg_ms"] * kernels[dom]["launches"] / total_kernel_ms,
-                "step_algo_bytes_per_update": step_bytes,
-                "step_achieved_gbs": value / world * step_bytes / 1e9,
-                "step_frac": value / world * step_bytes / 1e9 / peak,
-                "step_frac_of_8TBs_nominal": value / world * step_bytes / 1e9 / 8000.0,
-                "step_frac_of_16B_floor": value / world * 16 / 1e9 / peak,      # read C^n once, write C^{n+1} once
-                "note": ("achieved = algorithmic bytes / live CUDA-event time; a fraction above 1 means part of those bytes came from L2: "
-                         "consecutive kernels walk the ensemble in opposite directions, so each finds the tail of its predecessor's "
-                         "output in the 126 MB L2 (the ncu `traffic` figure is taken with caches flushed per launch)"),
-                "unfused_model_bytes_per_update": model_bytes,
-                "unfused_model_frac": value / world * model_bytes / 1e9 / peak}
+    roofline = None
+    if "step_resident" not in kernels:
+        main_kinds = {k: v for k, v in kernels.items() if not k.endswith("_diag")} or kernels
+        dom = max(main_kinds, key=lambda k: main_kinds[k]["avg_ms"] * main_kinds[k]["launches"])
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES.get((name, dom), (None, None))[0],
+                    "traffic_source": NCU_TRAFFIC_BYTES.get((name, dom), (None, None))[1],
+                    "peak_source": peak_src, "share_of_step": kernels[dom]["avg_ms"] * kernels[dom]["launches"] / total_kernel_ms,
+                    "step_algo_bytes_per_update": step_bytes,
+                    "step_achieved_gbs": value / world * step_bytes / 1e9,
+                    "step_frac": value / world * step_bytes / 1e9 / peak,
+                    "step_frac_of_8TBs_nominal": value / world * step_bytes / 1e9 / 8000.0,
+                    "step_frac_of_16B_floor": value / world * 16 / 1e9 / peak,      # read C^n once, write C^{n+1} once
+                    "note": ("achieved = algorithmic bytes / live CUDA-event time; a fraction above 1 means part of those bytes came from L2: "
+                             "consecutive kernels walk the ensemble in opposite directions, so each finds the tail of its predecessor's "
+                             "output in the 126 MB L2 (the ncu `traffic` figure is taken with caches flushed per launch)"),
+                    "unfused_model_bytes_per_update": model_bytes,
+                    "unfused_model_frac": value / world * model_bytes / 1e9 / peak}
+
+    if "step_resident" in kernels:
+        kr = kernels["step_resident"]
+        roofline = {"bound": "alu", "kernel": "step_resident", "achieved": kr["achieved_tinstr_s"], "peak": ALU_PEAK_TINSTR,
+                    "unit": "T fp64 instr/s", "frac": kr["frac"], "traffic": None, "traffic_source": None,
+                    "peak_source": "148 SMs x 64 fp64 lanes per clock (ncu sm__sass_thread_inst_executed_op_dfma peak_sustained) x 1.965 GHz, DESIGN.md 5c",
+                    "share_of_step": kr["avg_ms"] * kr["launches"] / total_kernel_ms,
+                    "step_algo_bytes_per_update": 16.0 / K, "step_frac_of_hbm_40B_structure": value / world * 40 / 1e9 / peak,
+                    "note": ("the members stay in shared memory for the whole call: HBM traffic is 16 B / K per update, and the fraction of "
+                             "the HBM roofline of the 40 B two-kernel structure this throughput would need is given for context (may exceed 1)")}
 
     # ---- paper-regime leg: same shape, gamma' = 66.4, dt' = 7.97 (sigma = 529, the
     # paper's gamma = 0.01, dx = 2 pi / 512, dt = 0.0012 in h = 1 units): the closure tables do not decay

@@ -52,10 +52,10 @@ def test_workspace_bytes_and_argument_errors(lib):
     assert b"ch_create" in lib.ch_last_error(None)
     assert lib.ch_destroy(None) == binding.CH_EINVAL
     assert lib.ch_step(None, 1) == binding.CH_EINVAL
-    assert lib.ch_kernel_kinds() == 11
-    assert [lib.ch_kernel_kind_name(k) for k in range(11)] == [b"rhs", b"rhs_diag", b"finish", b"sweep_x", b"sweep_y", b"sweep_z",
+    assert lib.ch_kernel_kinds() == 12
+    assert [lib.ch_kernel_kind_name(k) for k in range(12)] == [b"rhs", b"rhs_diag", b"finish", b"sweep_x", b"sweep_y", b"sweep_z",
                                                                 b"rhs_sweep_y", b"rhs_sweep_y_diag", b"sweep_x_update", b"sweep_xy",
-                                                                b"step_local"]
+                                                                b"step_local", b"step_resident"]
     d = ctypes.c_void_p()
     assert lib.ch_droplet_create(ctypes.byref(d), 0, 128, 1e-3) == binding.CH_EINVAL
     assert lib.ch_droplet_create(ctypes.byref(d), 4, 128, -1.0) == binding.CH_EINVAL

@@ -355,14 +355,15 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     tol, rtol = FIELD_TOL, SERIES_RTOL                      # also at gamma dt = 529
     e = B.Ensemble(M, N, 2, gamma, dt)
     cs, line, mode = B.ch_get_option(e.ctx, "fused"), B.ch_get_option(e.ctx, "line"), B.ch_get_option(e.ctx, "fuse_mode")
-    cline, local = B.ch_get_option(e.ctx, "cline"), B.ch_get_option(e.ctx, "local")
+    cline, local, res = B.ch_get_option(e.ctx, "cline"), B.ch_get_option(e.ctx, "local"), B.ch_get_option(e.ctx, "resident")
     e.close()
+    assert (res != 0) == (N in (32, 64, 96))                   # member-resident stepping: the member fits one CTA
     assert (local != 0) == (gamma == 1.0 and N >= 64)          # one-pass local step: small gamma dt only
     assert (cs == 0) == (N == 592)
     assert (line != 0) == (N in (32, 64, 96, 128, 160, 192, 224, 256, 320, 384, 448, 512))
     assert (cline != 0) == (N == 1024)                         # flag kernel at K <= 2, scan kernel in the paper regime
-    assert mode == (3 if line else (4 if cline else (5 if local else (2 if cs else 0))))
-    variants = [{"fuse": 1}] + ([{"fuse": 5}] if local else []) + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
+    assert mode == (6 if res else (3 if line else (4 if cline else (5 if local else (2 if cs else 0)))))
+    variants = [{"fuse": 1}] + ([{"fuse": 6}] if res else []) + ([{"fuse": 5}] if local else []) + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
         + ([{"fuse": 4}] if cline else [])
     for opts in variants:
         C, s = run_gpu(B, C0, gamma, dt, nsteps, 10, options=opts)
@@ -428,6 +429,60 @@ def test_flag_synchronised_kernels_are_deterministic_and_match_three_pass(B, M, 
     c, sc = run_gpu(B, C0, 1.0, 0.01, steps, 10, options=alt)
     assert np.abs(a - c).max() <= 1e-13
     assert_series_close(sa, sc, 1e-12)
+
+
+# ------------------------------------- member-resident stepping (one CTA per member; fuse = 6)
+@pytest.mark.parametrize("M,N,gamma,dt,nsteps,stride", [
+    (3, 32, 1.0, 0.01, 1000, 7), (2, 64, 1.0, 0.01, 1000, 50), (2, 96, 0.5, 0.02, 1000, 100),
+    (2, 64, 66.4, 7.97, 200, 10), (1, 96, 66.4, 7.97, 100, 1),         # gamma dt = 529: the full K-term closure
+])
+def test_resident_stepping_parity(B, oracle, M, N, gamma, dt, nsteps, stride):
+    """One launch per ch_step call, the member and its work array in shared memory for all its steps, the samples written
+    from inside the kernel: field and series against the oracle at the north star's depth, and bitwise against the same
+    job split into calls of 1, 0, n/2 - 1 and the remaining steps (samples at call boundaries are written once)."""
+    C0 = inputs.initial_state(range(50, 50 + M), N, 2, -0.2, 0.1)
+    e = B.Ensemble(M, N, 2, gamma, dt)
+    assert B.ch_get_option(e.ctx, "fuse_mode") == 6            # auto-selected
+    e.close()
+    C, s = run_gpu(B, C0, gamma, dt, nsteps, stride)
+    Co, so = oracle.run(C0, gamma, dt, nsteps, stride)
+    assert np.abs(C - Co).max() <= FIELD_TOL
+    assert_series_close(s, so)
+    e = B.Ensemble(M, N, 2, gamma, dt)
+    e.set_state(C0)
+    e.set_series(stride, nsteps // stride + 1)
+    for k in (1, 0, nsteps // 2 - 1, nsteps - nsteps // 2):
+        e.step(k)
+    assert B.ch_step_count(e.ctx) == nsteps and B.ch_series_count(e.ctx) == nsteps // stride + 1
+    C2, s2 = e.get_state(), e.series()
+    with pytest.raises(B.ChError):
+        e.step(stride)                                         # the series is full: refused, nothing enqueued
+    e.close()
+    assert np.array_equal(C, C2) and np.array_equal(s, s2)
+
+
+def test_resident_stepping_many_members_restart_and_determinism(B, oracle):
+    """More members than CTAs fit the device at once (700 x 64^2: three per SM), against the line kernel's step; a member's
+    result is bitwise independent of its position and of the ensemble around it; a restart with ch_set_time continues the
+    series of one uninterrupted run."""
+    C0 = inputs.initial_state(range(4000, 4700), 64, 2, -0.4, 0.05)
+    a, sa = run_gpu(B, C0, 1.0, 0.01, 60, 20)
+    b, sb = run_gpu(B, C0, 1.0, 0.01, 60, 20, options={"fuse": 3})
+    assert np.abs(a - b).max() <= 1e-13
+    assert_series_close(sa, sb, 1e-12)
+    r, sr = run_gpu(B, C0[::-1].copy(), 1.0, 0.01, 60, 20)
+    assert np.array_equal(r[::-1], a) and np.array_equal(sr[:, ::-1], sa)
+    one, s1 = run_gpu(B, C0[333:334].copy(), 1.0, 0.01, 60, 20)
+    assert np.array_equal(one[0], a[333]) and np.array_equal(s1[:, 0], sa[:, 333])
+    sub = [0, 333, 699]
+    Co, so = oracle.run(C0[sub], 1.0, 0.01, 60, 20)
+    assert np.abs(a[sub] - Co).max() <= FIELD_TOL
+    assert_series_close(sa[:, sub], so)
+    # restart: 40 steps, then a new context from that state at t0 = 40 dt for the last 20
+    h, _ = run_gpu(B, C0[:5].copy(), 1.0, 0.01, 40, 20)
+    c, sc = run_gpu(B, h, 1.0, 0.01, 20, 20, t0=40 * 0.01)
+    assert np.array_equal(c, a[:5])
+    assert_series_close(sc[1:], sa[3:, :5], 1e-14)
 
 
 # ------------------------------------- one-pass local step (SURVEY.md 8(f) NEXT-3 (i); option fuse = 5; DESIGN.md 5b)
@@ -591,6 +646,7 @@ def test_flag_synchronised_kernels_repeat_bitwise_under_load(B, M, N, steps):
     (6, 64, 3, 12, 4, 4, None),               # 3D
     (7, 352, 2, 15, 5, 3, None),              # one-pass local step (auto), odd number of steps: arrays end up swapped
     (3, 24, 2, 9, 3, 1, None),                # generic path
+    (11, 64, 2, 23, 5, 4, None),              # member-resident stepping (auto): one launch per chunk
 ])
 def test_run_host_is_set_state_step_get_state(B, M, N, D, nsteps, stride, chunk, opts):
     """ch_run_host (host -> chunk-pipelined H2D / steps / D2H on three streams -> host) against the plain
