@@ -351,7 +351,8 @@ def run_ours(args):
             "ms_per_step": secs / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_desc(name), "members_per_gpu": M, "options": opts, "fuse_mode": fuse_mode_used, "parallelism": f"ensemble-sharded x{world} (no data-path collective)",
-                       "l2": f"working set {2 * state_bytes >> 20} MiB per GPU, larger than the 126 MB L2; no explicit flush",
+                       "l2": (f"working set {2 * state_bytes >> 20} MiB per GPU, larger than the 126 MB L2; no explicit flush" if 2 * state_bytes > (126 << 20)
+                              else f"working set {2 * state_bytes >> 20} MiB per GPU: SMALLER than the 126 MB L2 and not flushed (a small-ensemble parity config, not the headline)"),
                        "sampling": (f"F, dF/dt, beta, mass every {stride} steps; {samples_in} sampling step(s) inside the {K}-step timed region "
                                     f"(every repetition starts at step n = {phase} mod {stride})")},
             "samples_in_timed_region": samples_in, "repetitions": repetitions,

@@ -164,11 +164,12 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *              update), legal when the recurrences of the factorisation decay within 18 points to below 2^-56 of the
  *              data (gamma dt <~ 0.012; the bound is computed on the host, "local_reach"); auto picks it for D = 2,
  *              N >= 256 when it is legal and the exact modes otherwise; 6 member-resident stepping (SURVEY.md 8(f)
- *              NEXT-3 (ii), one CTA per member; D = 2, N in {32, 64, 96}): a whole ch_step(nsteps) call, with the samples
+ *              NEXT-3 (ii); D = 2; one CTA per member for N in {32, 64, 96}, a cluster of 2 / 8 CTAs for N = 128 / 256):
+ *              a whole ch_step(nsteps) call, with the samples
  *              that fall inside it, is ONE launch that keeps each member and its work array in shared memory (exact
  *              periodic solves, any gamma dt; global memory is read and written once per call, so the bound is the
- *              fp64 / shared-memory pipe, not HBM); auto picks it wherever it is legal (measured 1.9 - 2.3 x the line
- *              kernel).  A mode the shape does not support is CH_EINVAL.
+ *              fp64 / shared-memory pipe, not HBM); auto picks it for N <= 128 (measured 1.1 - 2.3 x the line kernel;
+ *              at N = 256 it measures slower than the line kernel and is explicit only).  A mode the shape does not support is CH_EINVAL.
  *   "linesync" line kernel: 0 auto (neighbour-warp flags when the closure is truncated to 2 chunks), 1 CTA barriers
  *   "scan"     closure of the chunk states: 0 auto (log-depth shuffle scan when the K-term sum is long), 1 K-term
  *              sum always, 2 scan wherever it is available
@@ -180,8 +181,8 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  * ch_get_option answers these and, read-only: "chunked" (chunk length of the fast sweeps, 0 if N needs the generic
  * path), "K" (chunks summed by the periodic closure), "fused" / "line" / "cline" / "rhs3_stream" / "sweep_xy"
  * (non-zero if this shape has that kernel), "local" (non-zero if the one-pass local step is legal for this shape and
- * gamma dt), "local_reach" (its decay reach H in points, -1 if above the limit), "resident" (non-zero if member-resident
- * stepping is available for this shape), "fuse_mode" (the 2D step that will run: 0, 2, 3, 4, 5 or 6). */
+ * gamma dt), "local_reach" (its decay reach H in points, -1 if above the limit), "resident" (CTAs per member if member-resident
+ * stepping is available for this shape, else 0), "fuse_mode" (the 2D step that will run: 0, 2, 3, 4, 5 or 6). */
 int ch_set_option(ch_ctx *ctx, const char *key, int value);
 int ch_get_option(const ch_ctx *ctx, const char *key, int *value);
 

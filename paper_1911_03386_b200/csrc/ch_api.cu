@@ -89,6 +89,8 @@ struct ch_ctx {
     int loc_H, loc_resident;     // decay reach (ch_factor_reach), CTAs resident on the device
     // member-resident stepping: one CTA holds a member in shared memory for a whole ch_step call (ch_resident2d.cuh)
     bool resident_ok;
+    int res_clusters;            // clusters of that size resident on the device
+    int res_CS;                  // CTAs per member: 1 (N <= 96), else the cluster size (N = 128: 2, N = 256: 8)
     // ch_run_host: the kernels run on a member sub-range ("view"): M, total, C, w point at the view, these keep the whole
     int Mfull, view_m0;
     cudaStream_t rh_in, rh_comp, rh_out;     // its three internal streams (created on first use)
@@ -108,7 +110,9 @@ static int fuse_mode(const ch_ctx *c)
     if (c->opt_fuse == 6) return c->resident_ok ? 6 : 0;
     // auto: a member that fits one CTA's shared memory stays there for the whole ch_step call (measured on B200, 64^2: 3.3 vs 7.2 us
     // per step for one member, 2.7e11 vs 1.4e11 updates/s for 4096 members)
-    if (c->opt_fuse == 0 && c->resident_ok) return 6;
+    // (128^2 over 2-CTA clusters: 1.59e11 vs 0.92e11 - 1.45e11; 256^2 over 8-CTA clusters is SLOWER than the line kernel, 1.13e11 vs
+    // 1.40e11 -- 15 clusters fit the device and a CTA's phases do not overlap -- and stays an explicit option)
+    if (c->opt_fuse == 0 && c->resident_ok && c->res_CS <= 2) return 6;
     // auto: the line kernels where the shape has one (measured faster: CFG3 0.218 vs 0.263 ms); everywhere else the
     // one-pass local step when gamma dt allows it (N = 768: 0.274 vs 0.324 ms; N % 16 != 0: 0.25 vs 2.5 - 6.3 ms)
     if (c->opt_fuse == 0 && c->local_ok && !c->line_ok && !c->cline_ok) return 5;
@@ -119,6 +123,38 @@ static int fuse_mode(const ch_ctx *c)
 }
 
 static bool use_rhs3_stream(const ch_ctx *c) { return c->r3_ok && c->opt_rhs3 != 1; }
+
+// member-resident stepping over clusters: (N, CTAs per member) instantiated
+// (measured on B200, updates/s at 512 / 256 members: 128^2: 2 CTAs 1.59e11, 4 CTAs 1.41e11, 8 CTAs 1.44e11; 256^2: 8 CTAs 1.13e11, 16 CTAs 1.14e11)
+#define RES_CL_CASES(X) X(128, 2) X(256, 8)
+template <int NC, int CS>
+static void res_cl_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *at, int members, cudaStream_t st)
+{
+    cfg.gridDim = dim3((unsigned)members * CS); cfg.blockDim = dim3(NC * (NC / CS) / RES_LC);
+    cfg.dynamicSmemBytes = resident_cl_smem(NC, CS); cfg.stream = st;
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+}
+template <int NC, int CS>
+static cudaError_t res_cl_setup(int *nclusters)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_step2d_resident_cl<NC, CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)resident_cl_smem(NC, CS));
+    if (e == cudaSuccess && CS > 8) e = cudaFuncSetAttribute(k_step2d_resident_cl<NC, CS>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    res_cl_config<NC, CS>(cfg, at, 1, 0);
+    return cudaOccupancyMaxActiveClusters(nclusters, k_step2d_resident_cl<NC, CS>, &cfg);
+}
+template <int NC, int CS>
+static void res_cl_launch(ch_ctx *c, const SweepParams &prm, const ResidentParams &rp)
+{
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    res_cl_config<NC, CS>(cfg, at, c->M, c->stream);
+    cudaLaunchKernelEx(&cfg, k_step2d_resident_cl<NC, CS>, prm, rp, c->C);
+}
 
 // Brackets one kernel launch with CUDA events on the context's stream when profiling is on.
 struct ProfScope {
@@ -376,7 +412,18 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         }
     }
     // member-resident stepping: the member and its work array in one CTA's shared memory
-    c->resident_ok = false;
+    c->resident_ok = false; c->res_CS = 1;
+    if (D == 2 && c->LC == RES_LC && (N == 128 || N == 256)) {
+        c->res_CS = N == 128 ? 2 : 8;
+        int nclusters = 0;
+        cudaError_t e = cudaErrorInvalidValue;
+#define X(NC, CS) if (N == NC && c->res_CS == CS) e = res_cl_setup<NC, CS>(&nclusters);
+        RES_CL_CASES(X)
+#undef X
+        c->resident_ok = e == cudaSuccess && nclusters >= 1;
+        c->res_clusters = nclusters;
+        cudaGetLastError();
+    }
     if (D == 2 && c->LC == RES_LC && (N == 32 || N == 64 || N == 96)) {
         cudaError_t e = cudaSuccess;
         const int smem = (int)resident_smem(N);
@@ -597,7 +644,7 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
     }
     if (!strcmp(key, "fuse")) {
         if (value < 0 || value > 6) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line), 4 (cluster line), 5 (one-pass local) or 6 (member-resident)");
-        if (value == 6 && !ctx->resident_ok) return fail(ctx, CH_EINVAL, "ch_set_option: member-resident stepping needs D = 2 and N in {32, 64, 96}");
+        if (value == 6 && !ctx->resident_ok) return fail(ctx, CH_EINVAL, "ch_set_option: member-resident stepping needs D = 2 and N in {32, 64, 96, 128, 256}");
         if (value == 5 && !ctx->local_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the one-pass local step needs D = 2, N % 4 == 0 and a decay reach <= 18 points (gamma dt <~ 0.012)");
         if (value == 4 && !ctx->cline_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster line step needs D = 2 and N in {1024, 2048, 4096}");
         if (value == 2 && !ctx->fused_ok) return fail(ctx, CH_EINVAL, "ch_set_option: the cluster-fused step needs D = 2 and N % 16 == 0");
@@ -628,7 +675,8 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "fuse_mode")) { *value = fuse_mode(ctx); return CH_OK; }
     if (!strcmp(key, "local")) { *value = ctx->local_ok ? ctx->loc_resident : 0; return CH_OK; }
     if (!strcmp(key, "local_reach")) { *value = ctx->loc_H; return CH_OK; }
-    if (!strcmp(key, "resident")) { *value = ctx->resident_ok ? 1 : 0; return CH_OK; }
+    if (!strcmp(key, "resident")) { *value = ctx->resident_ok ? ctx->res_CS : 0; return CH_OK; }
+    if (!strcmp(key, "resident_clusters")) { *value = ctx->resident_ok ? ctx->res_clusters : 0; return CH_OK; }
     return CH_EINVAL;
 }
 
@@ -1021,8 +1069,12 @@ static void launch_step_resident(ch_ctx *c, int nsteps, double *energy_out = nul
     if (energy_out) {
         rp.nsteps = 0; rp.stride = 1; rp.last_sampled = -1; rp.cursor0 = 0; rp.Mfull = c->M; rp.view_m0 = 0; rp.series = energy_out;
     }
+#define X(NC, CS) if (c->N == NC && c->res_CS == CS) res_cl_launch<NC, CS>(c, prm, rp);
+    RES_CL_CASES(X)
+#undef X
     const size_t smem = resident_smem(c->N);
-    if (c->N == 32) k_step2d_resident<32><<<c->M, 32 * 32 / RES_LC, smem, c->stream>>>(prm, rp, c->C);
+    if (c->res_CS > 1) {}
+    else if (c->N == 32) k_step2d_resident<32><<<c->M, 32 * 32 / RES_LC, smem, c->stream>>>(prm, rp, c->C);
     else if (c->N == 64) k_step2d_resident<64><<<c->M, 64 * 64 / RES_LC, smem, c->stream>>>(prm, rp, c->C);
     else k_step2d_resident<96><<<c->M, 96 * 96 / RES_LC, smem, c->stream>>>(prm, rp, c->C);
     if (energy_out) return;

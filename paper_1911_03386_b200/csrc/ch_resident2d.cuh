@@ -1,5 +1,6 @@
-// ch_resident2d.cuh -- member-resident 2D stepping for members that fit one CTA's shared memory (N <= 96).
-// SURVEY.md section 8(f) NEXT-3 (ii), reduced to one CTA per member; DESIGN.md section 5c.
+// ch_resident2d.cuh -- member-resident 2D stepping: a member and its work array stay in shared memory for a whole ch_step call.
+// SURVEY.md section 8(f) NEXT-3 (ii); DESIGN.md section 5c.  One CTA per member for N <= 96 (first kernel), a thread-block
+// cluster per member for N = 128 (2 CTAs) and N = 256 (8 CTAs) (second kernel, end of this file).
 //
 //   k_step2d_resident   nsteps whole steps  C^{n+1} = C^n + A_x^-1 A_y^-1 dt Lap_h mu(C^n)
 //                       (+ the {F, dF/dt, beta, mass} samples that fall inside them)
@@ -122,4 +123,179 @@ __global__ void __launch_bounds__(NC * NC / RES_LC) k_step2d_resident(const __gr
         __syncthreads();
     }
     for (int i = tid; i < N * N; i += NT) Cm[i] = sC[(i / N) * PITCH + (i % N)];
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// The same for members that need the shared memory of a thread-block CLUSTER (N = 128: 2 CTAs, N = 256: 8 CTAs; the
+// "256^2 member + work array = 1 MiB in an 8-CTA cluster" of SURVEY.md 8(f) NEXT-3 (ii)).  CTA `rank` owns rows
+// rank * ROWS .. + ROWS - 1 (ROWS = N / CS) of C and w.  What crosses CTAs, all through distributed shared memory:
+//   - the C and mu rows just above / below a slab: every CTA PUSHES its first and last row into its neighbours' halo
+//     buffers (C after the update, mu in phase 1), so the stencils read local memory only;
+//   - the y-sweep's chunk out-states: written locally, PULLED by the K following (forward) / preceding (backward)
+//     chunks' owners after a cluster barrier (separate forward and backward slots: no barrier between the passes);
+//   - the per-CTA F, dF/dt, mass partials on sampling steps (pushed to rank 0, summed there in rank order).
+// x-lines lie inside a CTA (chunk_solve, CTA barriers).  Four cluster barriers per step (five on sampling steps).
+// ------------------------------------------------------------------------------------------------------------------
+#include <cooperative_groups.h>
+
+static inline size_t resident_cl_smem(int N, int CS)
+{
+    const size_t rows = N / CS, nt = (size_t)N * rows / RES_LC;
+    return ((size_t)2 * rows * (N + 1) + (size_t)4 * N + 6 * nt) * 8;
+}
+
+// grid = members * CS (cluster dimension CS), block = NC * (NC / CS) / 16, dynamic smem = resident_cl_smem(NC, CS)
+template <int NC, int CS>
+__global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_cl(const __grid_constant__ SweepParams prm,
+                                                                                     const __grid_constant__ ResidentParams rp,
+                                                                                     double *__restrict__ C)
+{
+    namespace cg = cooperative_groups;
+    constexpr int N = NC, LC = RES_LC, ROWS = NC / CS, PC = ROWS / LC, P = NC / LC, NT = NC * PC, PITCH = NC + 1, NW = NT / 32;
+    static_assert(ROWS % LC == 0 && NT % 32 == 0 && NT <= 1024, "slab geometry");
+    extern __shared__ double rsm[];
+    __shared__ double red[NW][3];
+    __shared__ double cpart[CS][3];
+    double *sC = rsm, *sw = sC + ROWS * PITCH, *hC = sw + ROWS * PITCH, *hM = hC + 2 * N;      // halos: [0] row above, [1] row below
+    double *yFa = hM + 2 * N, *yFb = yFa + NT, *yBa = yFb + NT, *yBb = yBa + NT, *xa = yBb + NT, *xb = xa + NT;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank(), prevR = (rank + CS - 1) % CS, nextR = (rank + 1) % CS;
+    const int tid = threadIdx.x, m = blockIdx.x / CS;
+    double *Cm = C + (size_t)m * N * N + (size_t)rank * ROWS * N;
+    // column mapping: column x, local chunk c (rows 16 c ..); row mapping: local row y, chunk cx (columns 16 cx ..)
+    const int x = tid % N, c = tid / N, r0 = c * LC, g = rank * PC + c;
+    const int y = tid % ROWS, cx = tid / ROWS, x0 = cx * LC;
+    const int xm = x == 0 ? N - 1 : x - 1, xp = x == N - 1 ? 0 : x + 1;
+    double *hC_prev = cluster.map_shared_rank(hC, prevR) + N, *hC_next = cluster.map_shared_rank(hC, nextR);   // my first row is prev's "below"
+    double *hM_prev = cluster.map_shared_rank(hM, prevR) + N, *hM_next = cluster.map_shared_rank(hM, nextR);
+
+    for (int i = tid; i < ROWS * N; i += NT) {
+        const int yy = i / N, xx = i % N;
+        const double v = Cm[i];
+        sC[yy * PITCH + xx] = v;
+        if (yy == 0) hC_prev[xx] = v;
+        if (yy == ROWS - 1) hC_next[xx] = v;
+    }
+    cluster.sync();
+
+    const double mgam = rp.mgam, k1 = rp.k1, scale = rp.scale, np = prm.np, nq = prm.nq;
+    int cursor = rp.cursor0;
+    for (int i = 0;; ++i) {
+        const long long n = rp.n0 + i;
+        const bool sample = rp.stride > 0 && n % rp.stride == 0 && n != rp.last_sampled;
+        const bool last = i == rp.nsteps;
+        if (last && !sample) break;
+        double F = 0.0, Fd = 0.0, ms = 0.0;
+        // ---- phase 1: mu -> w, edge rows also into the neighbours' halos
+        {
+            double cu = c == 0 ? hC[x] : sC[(r0 - 1) * PITCH + x], cc = sC[r0 * PITCH + x];
+#pragma unroll
+            for (int k = 0; k < LC; ++k) {
+                const int row = r0 + k;
+                const double cd = (k == LC - 1 && c == PC - 1) ? hC[N + x] : sC[(row + 1) * PITCH + x];
+                const double cl = sC[row * PITCH + xm], cr = sC[row * PITCH + xp];
+                const double mu = fma(mgam, (cl + cr) + (cu + cd), cc * fma(cc, cc, k1));
+                sw[row * PITCH + x] = mu;
+                if (k == 0 && c == 0) hM_prev[x] = mu;
+                if (k == LC - 1 && c == PC - 1) hM_next[x] = mu;
+                if (sample) {
+                    const double dx = cr - cc, dy = cd - cc, q = cc * cc - 1.0;
+                    F += 0.25 * q * q + 0.5 * rp.gamma * (dx * dx + dy * dy);
+                    ms += cc;
+                }
+                cu = cc; cc = cd;
+            }
+        }
+        cluster.sync();
+        // ---- phase 2: r = scale Lap_h mu
+        double v[LC];
+        {
+            double mu_u = c == 0 ? hM[x] : sw[(r0 - 1) * PITCH + x], mu_c = sw[r0 * PITCH + x];
+#pragma unroll
+            for (int k = 0; k < LC; ++k) {
+                const int row = r0 + k;
+                const double mu_d = (k == LC - 1 && c == PC - 1) ? hM[N + x] : sw[(row + 1) * PITCH + x];
+                const double ml = sw[row * PITCH + xm], mr = sw[row * PITCH + xp];
+                v[k] = scale * fma(-4.0, mu_c, (ml + mr) + (mu_u + mu_d));
+                if (sample) {
+                    const double dx = mr - mu_c, dy = mu_d - mu_c;
+                    Fd -= dx * dx + dy * dy;
+                }
+                mu_u = mu_c; mu_c = mu_d;
+            }
+        }
+        if (sample) {
+            block_sum3<NW>(F, Fd, ms, red);
+            if (tid == 0) {
+                double *o = cluster.map_shared_rank(&cpart[0][0], 0) + 3 * rank;
+                o[0] = F; o[1] = Fd; o[2] = ms;
+            }
+            cluster.sync();
+            if (rank == 0 && tid == 0) {
+                double f = cpart[0][0], fd = cpart[0][1], s = cpart[0][2];
+                for (int q = 1; q < CS; ++q) { f += cpart[q][0]; fd += cpart[q][1]; s += cpart[q][2]; }
+                const double t = rp.t0 + (double)n * rp.dt;
+                double *o = rp.series + ((size_t)cursor * rp.Mfull + rp.view_m0 + m) * 4;
+                o[0] = f; o[1] = fd; o[2] = (f == 0.0) ? 0.0 : -t * fd / f; o[3] = s;
+            }
+            ++cursor;
+        }
+        if (last) break;
+        __syncthreads();                     // every LOCAL mu read is done (the halos were pushed): w may be overwritten
+        // ---- phase 3: y-sweep, the line spread over the cluster
+        {
+            double a = 0.0, b = 0.0;
+            v[1] = fma(np, v[0], v[1]);
+#pragma unroll
+            for (int k = 2; k < LC; ++k) v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k]));
+            yFa[c * N + x] = v[LC - 1];
+            yFb[c * N + x] = v[LC - 2];
+            cluster.sync();
+            int s = g;
+            for (int j = 0; j < prm.K; ++j) {
+                s = s == 0 ? P - 1 : s - 1;
+                const int owner = s / PC, ls = s - owner * PC;
+                const double oa = cluster.map_shared_rank(yFa, owner)[ls * N + x], ob = cluster.map_shared_rank(yFb, owner)[ls * N + x];
+                const double2 W01 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j);
+                const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
+                a = fma(W01.x, oa, fma(W01.y, ob, a));
+                b = fma(W23.x, oa, fma(W23.y, ob, b));
+            }
+#pragma unroll
+            for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
+            v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
+#pragma unroll
+            for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
+            yBa[c * N + x] = v[0];
+            yBb[c * N + x] = v[1];
+            cluster.sync();
+            a = 0.0; b = 0.0; s = g;
+            for (int j = 0; j < prm.K; ++j) {
+                s = s == P - 1 ? 0 : s + 1;
+                const int owner = s / PC, ls = s - owner * PC;
+                const double oa = cluster.map_shared_rank(yBa, owner)[ls * N + x], ob = cluster.map_shared_rank(yBb, owner)[ls * N + x];
+                const double2 W01 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j);
+                const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
+                a = fma(W01.x, oa, fma(W01.y, ob, a));
+                b = fma(W23.x, oa, fma(W23.y, ob, b));
+            }
+#pragma unroll
+            for (int k = 0; k < LC; ++k) sw[(r0 + k) * PITCH + x] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
+        }
+        __syncthreads();
+        // ---- phase 4: x-sweep of local row y, columns x0 .. x0 + 15, the update, and the new edge rows into the neighbours' halos
+#pragma unroll
+        for (int k = 0; k < LC; ++k) v[k] = sw[y * PITCH + x0 + k];
+        chunk_solve<LC>(prm, v, xa + y, xb + y, cx, ROWS);
+#pragma unroll
+        for (int k = 0; k < LC; ++k) {
+            const double cn = sC[y * PITCH + x0 + k] + v[k];
+            sC[y * PITCH + x0 + k] = cn;
+            if (y == 0) hC_prev[x0 + k] = cn;
+            if (y == ROWS - 1) hC_next[x0 + k] = cn;
+        }
+        cluster.sync();
+    }
+    cluster.sync();                          // nobody leaves while a neighbour may still push into its halos
+    for (int i = tid; i < ROWS * N; i += NT) Cm[i] = sC[(i / N) * PITCH + (i % N)];
 }

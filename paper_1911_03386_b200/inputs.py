@@ -64,6 +64,9 @@ CONFIGS["n1000"] = dict(ensemble=32, N=1000, D=2, gamma=1.0, dt=0.01, nsteps=200
 # 3D shapes outside the streaming / plane-kernel sizes {64, 128} (they take the tile RHS + three separate sweeps, 72 B per update)
 CONFIGS["c96"] = dict(ensemble=38, N=96, D=3, gamma=1.0, dt=0.01, nsteps=10000, stride=50, cbar=-0.4, amp=0.05, seed0=7000)
 CONFIGS["c256"] = dict(ensemble=2, N=256, D=3, gamma=1.0, dt=0.01, nsteps=10000, stride=50, cbar=-0.4, amp=0.05, seed0=8000)
+# large ensembles of SMALL members (cfg1's 64^2, and 128^2): the shapes member-resident stepping serves; 2^22 points
+CONFIGS["r64"] = dict(ensemble=1024, N=64, D=2, gamma=1.0, dt=0.01, nsteps=5000, stride=50, cbar=0.0, amp=0.1, seed0=9000)
+CONFIGS["r128"] = dict(ensemble=256, N=128, D=2, gamma=1.0, dt=0.01, nsteps=5000, stride=50, cbar=-0.4, amp=0.05, seed0=10000)
 
 
 def config_state(name: str, members=None) -> np.ndarray:

@@ -357,12 +357,12 @@ def test_fused_and_three_pass_2d_paths(B, oracle, N, gamma, dt):
     cs, line, mode = B.ch_get_option(e.ctx, "fused"), B.ch_get_option(e.ctx, "line"), B.ch_get_option(e.ctx, "fuse_mode")
     cline, local, res = B.ch_get_option(e.ctx, "cline"), B.ch_get_option(e.ctx, "local"), B.ch_get_option(e.ctx, "resident")
     e.close()
-    assert (res != 0) == (N in (32, 64, 96))                   # member-resident stepping: the member fits one CTA
+    assert (res != 0) == (N in (32, 64, 96, 128, 256))         # member-resident stepping: one CTA, or a cluster of 2 / 8
     assert (local != 0) == (gamma == 1.0 and N >= 64)          # one-pass local step: small gamma dt only
     assert (cs == 0) == (N == 592)
     assert (line != 0) == (N in (32, 64, 96, 128, 160, 192, 224, 256, 320, 384, 448, 512))
     assert (cline != 0) == (N == 1024)                         # flag kernel at K <= 2, scan kernel in the paper regime
-    assert mode == (6 if res else (3 if line else (4 if cline else (5 if local else (2 if cs else 0)))))
+    assert mode == (6 if res and N <= 128 else (3 if line else (4 if cline else (5 if local else (2 if cs else 0)))))
     variants = [{"fuse": 1}] + ([{"fuse": 6}] if res else []) + ([{"fuse": 5}] if local else []) + ([{"fuse": 2}] if cs else []) + ([{"fuse": 3}, {"fuse": 3, "linesync": 1}, {"fuse": 3, "linesync": 1, "scan": 2}, {"fuse": 3, "scan": 1}] if line else []) \
         + ([{"fuse": 4}] if cline else [])
     for opts in variants:
@@ -435,6 +435,8 @@ def test_flag_synchronised_kernels_are_deterministic_and_match_three_pass(B, M, 
 @pytest.mark.parametrize("M,N,gamma,dt,nsteps,stride", [
     (3, 32, 1.0, 0.01, 1000, 7), (2, 64, 1.0, 0.01, 1000, 50), (2, 96, 0.5, 0.02, 1000, 100),
     (2, 64, 66.4, 7.97, 200, 10), (1, 96, 66.4, 7.97, 100, 1),         # gamma dt = 529: the full K-term closure
+    (2, 128, 1.0, 0.01, 1000, 50), (3, 256, 1.0, 0.01, 1000, 100),     # clusters of 2 and 8 CTAs per member
+    (2, 128, 66.4, 7.97, 200, 10), (1, 256, 66.4, 7.97, 100, 5),       # ... with chunk states pulled from every CTA of the cluster
 ])
 def test_resident_stepping_parity(B, oracle, M, N, gamma, dt, nsteps, stride):
     """One launch per ch_step call, the member and its work array in shared memory for all its steps, the samples written
@@ -442,13 +444,14 @@ def test_resident_stepping_parity(B, oracle, M, N, gamma, dt, nsteps, stride):
     job split into calls of 1, 0, n/2 - 1 and the remaining steps (samples at call boundaries are written once)."""
     C0 = inputs.initial_state(range(50, 50 + M), N, 2, -0.2, 0.1)
     e = B.Ensemble(M, N, 2, gamma, dt)
-    assert B.ch_get_option(e.ctx, "fuse_mode") == 6            # auto-selected
+    assert B.ch_get_option(e.ctx, "fuse_mode") == (6 if N <= 128 else 3)      # auto-selected up to N = 128
     e.close()
-    C, s = run_gpu(B, C0, gamma, dt, nsteps, stride)
+    opts = {"fuse": 6}
+    C, s = run_gpu(B, C0, gamma, dt, nsteps, stride, options=opts)
     Co, so = oracle.run(C0, gamma, dt, nsteps, stride)
     assert np.abs(C - Co).max() <= FIELD_TOL
     assert_series_close(s, so)
-    e = B.Ensemble(M, N, 2, gamma, dt)
+    e = B.Ensemble(M, N, 2, gamma, dt, options=opts)
     e.set_state(C0)
     e.set_series(stride, nsteps // stride + 1)
     for k in (1, 0, nsteps // 2 - 1, nsteps - nsteps // 2):
@@ -483,6 +486,18 @@ def test_resident_stepping_many_members_restart_and_determinism(B, oracle):
     c, sc = run_gpu(B, h, 1.0, 0.01, 20, 20, t0=40 * 0.01)
     assert np.array_equal(c, a[:5])
     assert_series_close(sc[1:], sa[3:, :5], 1e-14)
+
+
+def test_resident_stepping_cluster_waves(B):
+    """157 members of 128^2 on 2-CTA clusters: more clusters than fit the device at once (74), an odd count; against the
+    line kernel's step, and bitwise independent of the member order."""
+    C0 = inputs.initial_state(range(6000, 6157), 128, 2, -0.4, 0.05)
+    a, sa = run_gpu(B, C0, 1.0, 0.01, 30, 10)
+    b, sb = run_gpu(B, C0, 1.0, 0.01, 30, 10, options={"fuse": 3})
+    assert np.abs(a - b).max() <= 1e-13
+    assert_series_close(sa, sb, 1e-12)
+    r, sr = run_gpu(B, C0[::-1].copy(), 1.0, 0.01, 30, 10)
+    assert np.array_equal(r[::-1], a) and np.array_equal(sr[:, ::-1], sa)
 
 
 # ------------------------------------- one-pass local step (SURVEY.md 8(f) NEXT-3 (i); option fuse = 5; DESIGN.md 5b)
@@ -615,7 +630,7 @@ def test_flag_synchronised_kernels_repeat_bitwise_under_load(B, M, N, steps):
     import torch
     C0 = torch.from_numpy(inputs.initial_state(range(700, 700 + M), N, 2, -0.3, 0.1)).cuda()
     side, junk = torch.cuda.Stream(), torch.empty(32 << 20, dtype=torch.float32, device="cuda")
-    e = B.Ensemble(M, N, 2, 1.0, 0.01)
+    e = B.Ensemble(M, N, 2, 1.0, 0.01, options={"fuse": 3} if N <= 128 else None)
     assert B.ch_get_option(e.ctx, "fuse_mode") in (3, 4)
     ser = torch.empty((steps // 2 + 1, M, 4), dtype=torch.float64, device="cuda")
     ref = None
