@@ -172,13 +172,15 @@ def run_ours(args):
     name = args.workload
     c = inputs.CONFIGS[name]
     M, N, D, stride = c["ensemble"], c["N"], c["D"], c["stride"]
+    if args.members:                 # same recipe, another ensemble size (not a BASELINE.json config then)
+        M = args.members
     pts = M * N ** D
     K, W = args.steps, args.warmup
 
     # weak scaling: every rank steps its own full ensemble (disjoint seeds), no data-path collective
     seeds_off = rank * M
     cb = c["cbar"]
-    cbars = cb if isinstance(cb, (list, tuple)) else [cb] * M
+    cbars = [cb[k % len(cb)] for k in range(M)] if isinstance(cb, (list, tuple)) else [cb] * M
     host = torch.empty((M,) + (N,) * D, dtype=torch.float64).pin_memory()
     host.numpy()[...] = inputs.initial_state([c["seed0"] + seeds_off + k for k in range(M)], N, D, cbars, c["amp"])
     host_out = torch.empty_like(host).pin_memory()
@@ -350,7 +352,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": secs / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_desc(name), "members_per_gpu": M, "options": opts, "fuse_mode": fuse_mode_used, "parallelism": f"ensemble-sharded x{world} (no data-path collective)",
+            "config": {"workload": workload_desc(name) + (f" [--members {M}]" if args.members else ""), "members_per_gpu": M, "options": opts, "fuse_mode": fuse_mode_used, "parallelism": f"ensemble-sharded x{world} (no data-path collective)",
                        "l2": (f"working set {2 * state_bytes >> 20} MiB per GPU, larger than the 126 MB L2; no explicit flush" if 2 * state_bytes > (126 << 20)
                               else f"working set {2 * state_bytes >> 20} MiB per GPU: SMALLER than the 126 MB L2 and not flushed (a small-ensemble parity config, not the headline)"),
                        "sampling": (f"F, dF/dt, beta, mass every {stride} steps; {samples_in} sampling step(s) inside the {K}-step timed region "
@@ -375,6 +377,7 @@ def main():
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed K-step region (median reported)")
     ap.add_argument("--option", action="append", default=[], metavar="KEY=INT",
                     help="kernel-variant option passed to ch_set_option (include/ch.h), e.g. fuse=5; repeatable")
+    ap.add_argument("--members", type=int, default=0, help="override the ensemble size of the workload (same recipe and seeds)")
     ap.add_argument("--no-paper-regime", dest="paper_regime", action="store_false",
                     help="skip the extra timed leg at the paper's gamma dt / h^4 = 529")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (for runs under ncu)")
