@@ -170,6 +170,9 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *              periodic solves, any gamma dt; global memory is read and written once per call, so the bound is the
  *              fp64 / shared-memory pipe, not HBM); auto picks it for N <= 128 (measured 1.1 - 2.3 x the line kernel;
  *              at N = 256 it measures slower than the line kernel and is explicit only).  A mode the shape does not support is CH_EINVAL.
+ *   "resident_lines" one-CTA member-resident kernel (N <= 96): 0 auto (two lines per thread when at least two CTAs share an SM, i.e.
+ *              ensemble >= 2 x multiprocessors, or N = 96), 1 one line per thread, 2 two lines per thread (half the shared-
+ *              memory traffic, half the warps); fields and samples are bitwise the same either way
  *   "linesync" line kernel: 0 auto (neighbour-warp flags when the closure is truncated to 2 chunks), 1 CTA barriers
  *   "scan"     closure of the chunk states: 0 auto (log-depth shuffle scan when the K-term sum is long), 1 K-term
  *              sum always, 2 scan wherever it is available

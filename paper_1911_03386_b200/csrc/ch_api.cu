@@ -90,6 +90,8 @@ struct ch_ctx {
     // member-resident stepping: one CTA holds a member in shared memory for a whole ch_step call (ch_resident2d.cuh)
     bool resident_ok;
     int res_clusters;            // clusters of that size resident on the device
+    int sms;                     // multiprocessors of the device
+    int opt_resident;            // one-CTA kernel: 0 auto, 1 one line per thread, 2 two lines per thread
     int res_CS;                  // CTAs per member: 1 (N <= 96), else the cluster size (N = 128: 2, N = 256: 8)
     // ch_run_host: the kernels run on a member sub-range ("view"): M, total, C, w point at the view, these keep the whole
     int Mfull, view_m0;
@@ -412,7 +414,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         }
     }
     // member-resident stepping: the member and its work array in one CTA's shared memory
-    c->resident_ok = false; c->res_CS = 1;
+    c->resident_ok = false; c->res_CS = 1; c->sms = 1; c->opt_resident = 0;
     if (D == 2 && c->LC == RES_LC && (N == 128 || N == 256)) {
         c->res_CS = N == 128 ? 2 : 8;
         int nclusters = 0;
@@ -430,6 +432,13 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         if (N == 32) e = cudaFuncSetAttribute(k_step2d_resident<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         else if (N == 64) e = cudaFuncSetAttribute(k_step2d_resident<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         else e = cudaFuncSetAttribute(k_step2d_resident<96>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const int smem2 = (int)resident2_smem(N);
+        if (e == cudaSuccess && N == 32) e = cudaFuncSetAttribute(k_step2d_resident2<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+        if (e == cudaSuccess && N == 64) e = cudaFuncSetAttribute(k_step2d_resident2<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+        if (e == cudaSuccess && N == 96) e = cudaFuncSetAttribute(k_step2d_resident2<96>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2);
+        int dev = 0;
+        if (e == cudaSuccess) e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
         c->resident_ok = e == cudaSuccess;
         cudaGetLastError();
     }
@@ -642,6 +651,11 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_linesync = value;
         return CH_OK;
     }
+    if (!strcmp(key, "resident_lines")) {
+        if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: resident_lines must be 0 (auto), 1 (one line per thread) or 2 (two lines per thread)");
+        ctx->opt_resident = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "fuse")) {
         if (value < 0 || value > 6) return fail(ctx, CH_EINVAL, "ch_set_option: fuse must be 0 (auto), 1 (off), 2 (cluster), 3 (line), 4 (cluster line), 5 (one-pass local) or 6 (member-resident)");
         if (value == 6 && !ctx->resident_ok) return fail(ctx, CH_EINVAL, "ch_set_option: member-resident stepping needs D = 2 and N in {32, 64, 96, 128, 256}");
@@ -676,6 +690,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "local")) { *value = ctx->local_ok ? ctx->loc_resident : 0; return CH_OK; }
     if (!strcmp(key, "local_reach")) { *value = ctx->loc_H; return CH_OK; }
     if (!strcmp(key, "resident")) { *value = ctx->resident_ok ? ctx->res_CS : 0; return CH_OK; }
+    if (!strcmp(key, "resident_lines")) { *value = ctx->opt_resident; return CH_OK; }
     if (!strcmp(key, "resident_clusters")) { *value = ctx->resident_ok ? ctx->res_clusters : 0; return CH_OK; }
     return CH_EINVAL;
 }
@@ -1054,6 +1069,16 @@ static void launch_step_local(ch_ctx *c)
 static long long samples_ahead(const ch_ctx *ctx, int nsteps);
 
 // nsteps steps of the members in view, and the samples that fall inside them, in ONE launch (ch_resident2d.cuh)
+// Which one-CTA kernel: the two-lines-per-thread version moves half the shared-memory bytes but runs half the warps; it wins as soon as
+// several CTAs share an SM (64^2: 4096 members 3.39e11 vs 2.71e11 updates/s, 444 members 3.22e11 vs 2.59e11) and loses when a CTA has
+// an SM to itself (148 members: 1.58e11 vs 1.82e11; one member 3.5 vs 3.3 us per step); 96^2 has one CTA per SM either way (2.26e11 vs 2.01e11)
+static bool resident_two_lines(const ch_ctx *c)
+{
+    if (c->opt_resident == 1) return false;
+    if (c->opt_resident == 2) return true;
+    return c->N == 96 || c->M >= 2 * c->sms;
+}
+
 // energy_out != NULL: no steps, only {F, dF/dt, beta, mass} of the current state into energy_out[M][4] -- the same reduction,
 // in the same order, as the samples written from inside a stepping launch (ch_energy equals the series entry bitwise)
 static void launch_step_resident(ch_ctx *c, int nsteps, double *energy_out = nullptr)
@@ -1074,6 +1099,12 @@ static void launch_step_resident(ch_ctx *c, int nsteps, double *energy_out = nul
 #undef X
     const size_t smem = resident_smem(c->N);
     if (c->res_CS > 1) {}
+    else if (resident_two_lines(c)) {
+        const size_t smem2 = resident2_smem(c->N);
+        if (c->N == 32) k_step2d_resident2<32><<<c->M, 16 * 2, smem2, c->stream>>>(prm, rp, c->C);
+        else if (c->N == 64) k_step2d_resident2<64><<<c->M, 32 * 4, smem2, c->stream>>>(prm, rp, c->C);
+        else k_step2d_resident2<96><<<c->M, 48 * 6, smem2, c->stream>>>(prm, rp, c->C);
+    }
     else if (c->N == 32) k_step2d_resident<32><<<c->M, 32 * 32 / RES_LC, smem, c->stream>>>(prm, rp, c->C);
     else if (c->N == 64) k_step2d_resident<64><<<c->M, 64 * 64 / RES_LC, smem, c->stream>>>(prm, rp, c->C);
     else k_step2d_resident<96><<<c->M, 96 * 96 / RES_LC, smem, c->stream>>>(prm, rp, c->C);

@@ -31,6 +31,21 @@ struct ResidentParams {
     double *series;
 };
 
+// Diagnostics terms of one point, with every rounding spelled out (no compiler contraction), so that the kernels of this file, which
+// distribute the points over threads differently, add up the same numbers:
+//   F term = (c^2 - 1)^2 / 4 + gamma / 2 ((c_right - c)^2 + (c_down - c)^2)     P:34 eq. (4), readings G3, G4
+//   dissipation term = (mu_right - mu)^2 + (mu_down - mu)^2                      reading G5
+__device__ __forceinline__ double res_F_term(double c, double c_right, double c_down, double gamma)
+{
+    const double dx = __dsub_rn(c_right, c), dy = __dsub_rn(c_down, c), q = __fma_rn(c, c, -1.0);
+    return __fma_rn(__dmul_rn(0.25, q), q, __dmul_rn(__dmul_rn(0.5, gamma), __fma_rn(dx, dx, __dmul_rn(dy, dy))));
+}
+__device__ __forceinline__ double res_D_term(double mu, double mu_right, double mu_down)
+{
+    const double dx = __dsub_rn(mu_right, mu), dy = __dsub_rn(mu_down, mu);
+    return __fma_rn(dx, dx, __dmul_rn(dy, dy));
+}
+
 static inline size_t resident_smem(int N)
 {
     return ((size_t)2 * N * (N + 1) + (size_t)2 * (N / RES_LC) * N) * 8;
@@ -73,9 +88,8 @@ __global__ void __launch_bounds__(NC * NC / RES_LC) k_step2d_resident(const __gr
                 const double cl = sC[row * PITCH + xm], cr = sC[row * PITCH + xp];
                 sw[row * PITCH + j] = fma(mgam, (cl + cr) + (cu + cd), cc * fma(cc, cc, k1));
                 if (sample) {
-                    const double dx = cr - cc, dy = cd - cc, q = cc * cc - 1.0;
-                    F += 0.25 * q * q + 0.5 * rp.gamma * (dx * dx + dy * dy);
-                    ms += cc;
+                    F = __dadd_rn(F, res_F_term(cc, cr, cd, rp.gamma));
+                    ms = __dadd_rn(ms, cc);
                 }
                 cu = cc; cc = cd;
             }
@@ -91,10 +105,7 @@ __global__ void __launch_bounds__(NC * NC / RES_LC) k_step2d_resident(const __gr
                 const double mu_d = sw[(k == LC - 1 ? rn : row + 1) * PITCH + j];
                 const double ml = sw[row * PITCH + xm], mr = sw[row * PITCH + xp];
                 v[k] = scale * fma(-4.0, mu_c, (ml + mr) + (mu_u + mu_d));
-                if (sample) {
-                    const double dx = mr - mu_c, dy = mu_d - mu_c;
-                    Fd -= dx * dx + dy * dy;
-                }
+                if (sample) Fd = __dsub_rn(Fd, res_D_term(mu_c, mr, mu_d));
                 mu_u = mu_c; mu_c = mu_d;
             }
         }
@@ -199,9 +210,8 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
                 if (k == 0 && c == 0) hM_prev[x] = mu;
                 if (k == LC - 1 && c == PC - 1) hM_next[x] = mu;
                 if (sample) {
-                    const double dx = cr - cc, dy = cd - cc, q = cc * cc - 1.0;
-                    F += 0.25 * q * q + 0.5 * rp.gamma * (dx * dx + dy * dy);
-                    ms += cc;
+                    F = __dadd_rn(F, res_F_term(cc, cr, cd, rp.gamma));
+                    ms = __dadd_rn(ms, cc);
                 }
                 cu = cc; cc = cd;
             }
@@ -217,10 +227,7 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
                 const double mu_d = (k == LC - 1 && c == PC - 1) ? hM[N + x] : sw[(row + 1) * PITCH + x];
                 const double ml = sw[row * PITCH + xm], mr = sw[row * PITCH + xp];
                 v[k] = scale * fma(-4.0, mu_c, (ml + mr) + (mu_u + mu_d));
-                if (sample) {
-                    const double dx = mr - mu_c, dy = mu_d - mu_c;
-                    Fd -= dx * dx + dy * dy;
-                }
+                if (sample) Fd = __dsub_rn(Fd, res_D_term(mu_c, mr, mu_d));
                 mu_u = mu_c; mu_c = mu_d;
             }
         }
@@ -298,4 +305,187 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
     }
     cluster.sync();                          // nobody leaves while a neighbour may still push into its halos
     for (int i = tid; i < ROWS * N; i += NT) Cm[i] = sC[(i / N) * PITCH + (i % N)];
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Second version of the one-CTA kernel, built for the shared-memory data pipe that bounds the first (80 % busy, 106 B
+// per update): a thread owns TWO lines in every phase, so that
+//   - in the column mapping (columns 2 i, 2 i + 1) one of the two x-neighbours of every point is the thread's own
+//     value: 4 LDS per row pair instead of 6, and mu stays in registers between phases 1 and 2 (2 LDS instead of 6);
+//   - in the row mapping (rows y, y + N/2) the thread keeps its 2 x 16 values of C in REGISTERS for the whole launch:
+//     the update needs no load of C.
+// About 57 B per update through the data pipe.  Even and odd columns live in separate planes ([row][N/2 + 1], odd
+// pitch), so that both mappings stay bank-conflict free with 8-byte accesses.
+// ------------------------------------------------------------------------------------------------------------------
+static inline size_t resident2_smem(int N)
+{
+    return ((size_t)4 * N * (N / 2 + 1) + (size_t)2 * (N / RES_LC) * N) * 8;
+}
+
+// the exact periodic solve of chunk_solve (ch_kernels.cuh) for two lines at once (shared barriers); slots [chunk][line]
+template <int LC>
+__device__ __forceinline__ void chunk_solve_pair(const SweepParams &prm, double (&u)[LC], double (&v)[LC], double *sa, double *sb,
+                                                 int c, int stride, int i1, int i2)
+{
+    const double np = prm.np, nq = prm.nq;
+    const int P = prm.P;
+    auto state_in = [&](int dir, double &a1, double &b1, double &a2, double &b2) {
+        a1 = b1 = a2 = b2 = 0.0;
+        int s = c;
+        for (int j = 0; j < prm.K; ++j) {
+            s -= dir;
+            if (s < 0) s += P;
+            if (s >= P) s -= P;
+            const double2 W01 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j);
+            const double2 W23 = __ldg(reinterpret_cast<const double2 *>(prm.W) + 2 * j + 1);
+            const double oa1 = sa[s * stride + i1], ob1 = sb[s * stride + i1], oa2 = sa[s * stride + i2], ob2 = sb[s * stride + i2];
+            a1 = fma(W01.x, oa1, fma(W01.y, ob1, a1)); b1 = fma(W23.x, oa1, fma(W23.y, ob1, b1));
+            a2 = fma(W01.x, oa2, fma(W01.y, ob2, a2)); b2 = fma(W23.x, oa2, fma(W23.y, ob2, b2));
+        }
+    };
+    double a1, b1, a2, b2;
+    u[1] = fma(np, u[0], u[1]); v[1] = fma(np, v[0], v[1]);
+#pragma unroll
+    for (int k = 2; k < LC; ++k) { u[k] = fma(np, u[k - 1], fma(nq, u[k - 2], u[k])); v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k])); }
+    sa[c * stride + i1] = u[LC - 1]; sb[c * stride + i1] = u[LC - 2];
+    sa[c * stride + i2] = v[LC - 1]; sb[c * stride + i2] = v[LC - 2];
+    __syncthreads();
+    state_in(+1, a1, b1, a2, b2);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) { u[k] = fma(prm.alpha[k], a1, fma(prm.beta[k], b1, u[k])); v[k] = fma(prm.alpha[k], a2, fma(prm.beta[k], b2, v[k])); }
+    __syncthreads();
+    u[LC - 2] = fma(np, u[LC - 1], u[LC - 2]); v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
+#pragma unroll
+    for (int k = LC - 3; k >= 0; --k) { u[k] = fma(np, u[k + 1], fma(nq, u[k + 2], u[k])); v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k])); }
+    sa[c * stride + i1] = u[0]; sb[c * stride + i1] = u[1];
+    sa[c * stride + i2] = v[0]; sb[c * stride + i2] = v[1];
+    __syncthreads();
+    state_in(-1, a1, b1, a2, b2);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) {
+        u[k] = fma(prm.alpha[LC - 1 - k], a1, fma(prm.beta[LC - 1 - k], b1, u[k]));
+        v[k] = fma(prm.alpha[LC - 1 - k], a2, fma(prm.beta[LC - 1 - k], b2, v[k]));
+    }
+}
+
+// grid = members, block = (NC / 2) * (NC / 16), dynamic smem = resident2_smem(NC); C is updated in place
+template <int NC>
+__global__ void __launch_bounds__((NC / 2) * (NC / RES_LC), NC <= 64 ? 3 : 1) k_step2d_resident2(const __grid_constant__ SweepParams prm,
+                                                                                                 const __grid_constant__ ResidentParams rp,
+                                                                                                 double *__restrict__ C)
+{
+    constexpr int N = NC, LC = RES_LC, P = NC / LC, H = NC / 2, NT = H * P, PT = H + 1, NG = NT / 16;
+    static_assert(NT % 32 == 0, "whole warps");
+    extern __shared__ double rsm[];
+    __shared__ double red[NG][3];
+    double *sCE = rsm, *sCO = sCE + N * PT, *swE = sCO + N * PT, *swO = swE + N * PT, *sa = swO + N * PT, *sb = sa + P * N;
+    const int tid = threadIdx.x, ih = tid % H, c = tid / H, m = blockIdx.x;
+    double *Cm = C + (size_t)m * N * N;
+    // row mapping: rows y1 = ih and y2 = ih + H, columns 16 c .. 16 c + 15; their C values stay in registers
+    const int y1 = ih, y2 = ih + H, x0 = c * LC;
+    double C1[LC], C2[LC];
+    for (int i = tid; i < N * H; i += NT) {
+        const int yy = i / H, ii = i - yy * H;
+        const double2 v2 = *reinterpret_cast<const double2 *>(Cm + (size_t)yy * N + 2 * ii);
+        sCE[yy * PT + ii] = v2.x; sCO[yy * PT + ii] = v2.y;
+    }
+#pragma unroll
+    for (int k = 0; k < LC; ++k) { C1[k] = Cm[(size_t)y1 * N + x0 + k]; C2[k] = Cm[(size_t)y2 * N + x0 + k]; }
+    __syncthreads();
+
+    const double mgam = rp.mgam, k1 = rp.k1, scale = rp.scale;
+    // column mapping: columns A = 2 ih (even plane, index ih) and B = 2 ih + 1 (odd plane, index ih), rows r0 .. r0 + 15
+    const int im = ih == 0 ? H - 1 : ih - 1, ip = ih == H - 1 ? 0 : ih + 1;      // odd-plane index left of A, even-plane index right of B
+    const int r0 = c * LC, rm = r0 == 0 ? N - 1 : r0 - 1, rn = r0 + LC == N ? 0 : r0 + LC;
+    int cursor = rp.cursor0;
+
+    for (int i = 0;; ++i) {
+        const long long n = rp.n0 + i;
+        const bool sample = rp.stride > 0 && n % rp.stride == 0 && n != rp.last_sampled;
+        const bool last = i == rp.nsteps;
+        if (last && !sample) break;
+        // diagnostics are summed per COLUMN and combined in the order of the one-line kernel's shuffle tree (even columns, odd columns,
+        // then 32-column groups in order), so a sample does not depend on which of the two kernels the ensemble size selects
+        double FA = 0.0, FB = 0.0, FdA = 0.0, FdB = 0.0, msA = 0.0, msB = 0.0;
+        double vA[LC], vB[LC];
+        // ---- phase 1: mu of the 2 x 16 points -> registers and w
+        {
+            double cuA = sCE[rm * PT + ih], cuB = sCO[rm * PT + ih], ccA = sCE[r0 * PT + ih], ccB = sCO[r0 * PT + ih];
+#pragma unroll
+            for (int k = 0; k < LC; ++k) {
+                const int row = r0 + k, rd = k == LC - 1 ? rn : row + 1;
+                const double cdA = sCE[rd * PT + ih], cdB = sCO[rd * PT + ih];
+                const double cl = sCO[row * PT + im], cr = sCE[row * PT + ip];
+                vA[k] = fma(mgam, (cl + ccB) + (cuA + cdA), ccA * fma(ccA, ccA, k1));
+                vB[k] = fma(mgam, (ccA + cr) + (cuB + cdB), ccB * fma(ccB, ccB, k1));
+                swE[row * PT + ih] = vA[k]; swO[row * PT + ih] = vB[k];
+                if (sample) {
+                    FA = __dadd_rn(FA, res_F_term(ccA, ccB, cdA, rp.gamma)); msA = __dadd_rn(msA, ccA);
+                    FB = __dadd_rn(FB, res_F_term(ccB, cr, cdB, rp.gamma)); msB = __dadd_rn(msB, ccB);
+                }
+                cuA = ccA; ccA = cdA; cuB = ccB; ccB = cdB;
+            }
+        }
+        __syncthreads();
+        // ---- phase 2: r = scale Lap_h mu, in place (own mu from registers, x-neighbours and the two edge rows from w)
+        {
+            double upA = swE[rm * PT + ih], upB = swO[rm * PT + ih];
+            const double dnA = swE[rn * PT + ih], dnB = swO[rn * PT + ih];
+#pragma unroll
+            for (int k = 0; k < LC; ++k) {
+                const int row = r0 + k;
+                const double ml = swO[row * PT + im], mr = swE[row * PT + ip];
+                const double mA = vA[k], mB = vB[k];
+                const double mdA = k == LC - 1 ? dnA : vA[k + 1], mdB = k == LC - 1 ? dnB : vB[k + 1];
+                vA[k] = scale * fma(-4.0, mA, (ml + mB) + (upA + mdA));
+                vB[k] = scale * fma(-4.0, mB, (mA + mr) + (upB + mdB));
+                if (sample) {
+                    FdA = __dsub_rn(FdA, res_D_term(mA, mB, mdA));
+                    FdB = __dsub_rn(FdB, res_D_term(mB, mr, mdB));
+                }
+                upA = mA; upB = mB;
+            }
+        }
+        if (sample) {
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) {
+                FA += __shfl_down_sync(0xffffffffu, FA, o, 16); FB += __shfl_down_sync(0xffffffffu, FB, o, 16);
+                FdA += __shfl_down_sync(0xffffffffu, FdA, o, 16); FdB += __shfl_down_sync(0xffffffffu, FdB, o, 16);
+                msA += __shfl_down_sync(0xffffffffu, msA, o, 16); msB += __shfl_down_sync(0xffffffffu, msB, o, 16);
+            }
+            if ((tid & 15) == 0) { red[tid >> 4][0] = FA + FB; red[tid >> 4][1] = FdA + FdB; red[tid >> 4][2] = msA + msB; }
+            __syncthreads();
+            if (tid == 0) {
+                double F = red[0][0], Fd = red[0][1], ms = red[0][2];
+                for (int q = 1; q < NG; ++q) { F += red[q][0]; Fd += red[q][1]; ms += red[q][2]; }
+                const double t = rp.t0 + (double)n * rp.dt;
+                double *o = rp.series + ((size_t)cursor * rp.Mfull + rp.view_m0 + m) * 4;
+                o[0] = F; o[1] = Fd; o[2] = (F == 0.0) ? 0.0 : -t * Fd / F; o[3] = ms;
+            }
+            ++cursor;
+        }
+        if (last) break;
+        __syncthreads();                     // every mu has been read: w may be overwritten
+        // ---- phase 3: y-sweep of the two columns
+        chunk_solve_pair<LC>(prm, vA, vB, sa, sb, c, N, 2 * ih, 2 * ih + 1);
+#pragma unroll
+        for (int k = 0; k < LC; ++k) { swE[(r0 + k) * PT + ih] = vA[k]; swO[(r0 + k) * PT + ih] = vB[k]; }
+        __syncthreads();
+        // ---- phase 4: x-sweep of rows y1, y2 (columns x0 .. x0 + 15) and the update of the register copy and of the planes
+#pragma unroll
+        for (int k = 0; k < LC; ++k) {
+            const double *pl = (k & 1) ? swO : swE;
+            vA[k] = pl[y1 * PT + (x0 + k) / 2]; vB[k] = pl[y2 * PT + (x0 + k) / 2];
+        }
+        chunk_solve_pair<LC>(prm, vA, vB, sa, sb, c, N, y1, y2);
+#pragma unroll
+        for (int k = 0; k < LC; ++k) {
+            double *pl = (k & 1) ? sCO : sCE;
+            C1[k] += vA[k]; C2[k] += vB[k];
+            pl[y1 * PT + (x0 + k) / 2] = C1[k]; pl[y2 * PT + (x0 + k) / 2] = C2[k];
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int k = 0; k < LC; ++k) { Cm[(size_t)y1 * N + x0 + k] = C1[k]; Cm[(size_t)y2 * N + x0 + k] = C2[k]; }
 }

@@ -488,6 +488,20 @@ def test_resident_stepping_many_members_restart_and_determinism(B, oracle):
     assert_series_close(sc[1:], sa[3:, :5], 1e-14)
 
 
+@pytest.mark.parametrize("M,N", [(3, 32), (5, 64), (2, 96)])
+def test_resident_stepping_one_and_two_lines_per_thread_agree_bitwise(B, M, N):
+    """The two one-CTA kernels (one line per thread; two lines per thread, half the shared-memory traffic -- picked when CTAs share
+    an SM) do the same arithmetic per point and combine the diagnostics in the same order: fields AND samples are bitwise equal,
+    so a member's series does not depend on the ensemble size that selects the kernel."""
+    C0 = inputs.initial_state(range(80, 80 + M), N, 2, -0.3, 0.2)
+    a, sa = run_gpu(B, C0, 1.0, 0.01, 40, 4, options={"fuse": 6, "resident_lines": 1})
+    b, sb = run_gpu(B, C0, 1.0, 0.01, 40, 4, options={"fuse": 6, "resident_lines": 2})
+    assert np.array_equal(a, b) and np.array_equal(sa, sb)
+    a, sa = run_gpu(B, C0, 66.4, 7.97, 20, 5, options={"fuse": 6, "resident_lines": 1})
+    b, sb = run_gpu(B, C0, 66.4, 7.97, 20, 5, options={"fuse": 6, "resident_lines": 2})
+    assert np.array_equal(a, b) and np.array_equal(sa, sb)
+
+
 def test_resident_stepping_cluster_waves(B):
     """157 members of 128^2 on 2-CTA clusters: more clusters than fit the device at once (74), an odd count; against the
     line kernel's step, and bitwise independent of the member order."""
