@@ -46,9 +46,38 @@ __device__ __forceinline__ double res_D_term(double mu, double mu_right, double 
     return __fma_rn(dx, dx, __dmul_rn(dy, dy));
 }
 
+// The exact periodic solve of chunk_solve (ch_kernels.cuh) with SEPARATE exchange slots for the forward (fa, fb) and the backward
+// (ba, bb) pass: two CTA barriers per sweep instead of three.  Slots are [chunk * stride + line].  The first barrier also orders
+// everything the CTA did before the sweep against everything after it.
+template <int LC>
+__device__ __forceinline__ void res_chunk_solve(const SweepParams &prm, double (&v)[LC], double *fa, double *fb, double *ba, double *bb,
+                                                int c, int stride, int line)
+{
+    const double np = prm.np, nq = prm.nq;
+    double a, b;
+    v[1] = fma(np, v[0], v[1]);
+#pragma unroll
+    for (int k = 2; k < LC; ++k) v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k]));
+    fa[c * stride + line] = v[LC - 1];
+    fb[c * stride + line] = v[LC - 2];
+    __syncthreads();
+    chunk_state_in<LC>(prm, fa + line, fb + line, c, stride, +1, a, b);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[k], a, fma(prm.beta[k], b, v[k]));
+    v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
+#pragma unroll
+    for (int k = LC - 3; k >= 0; --k) v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k]));
+    ba[c * stride + line] = v[0];
+    bb[c * stride + line] = v[1];
+    __syncthreads();
+    chunk_state_in<LC>(prm, ba + line, bb + line, c, stride, -1, a, b);
+#pragma unroll
+    for (int k = 0; k < LC; ++k) v[k] = fma(prm.alpha[LC - 1 - k], a, fma(prm.beta[LC - 1 - k], b, v[k]));
+}
+
 static inline size_t resident_smem(int N)
 {
-    return ((size_t)2 * N * (N + 1) + (size_t)2 * (N / RES_LC) * N) * 8;
+    return ((size_t)2 * N * (N + 1) + (size_t)4 * (N / RES_LC) * N) * 8;
 }
 
 // grid = members, block = NC * NC / 16, dynamic smem = resident_smem(NC); C is updated in place
@@ -60,7 +89,7 @@ __global__ void __launch_bounds__(NC * NC / RES_LC) k_step2d_resident(const __gr
     constexpr int N = NC, LC = RES_LC, P = NC / LC, NT = NC * P, PITCH = NC + 1, NW = (NT + 31) / 32;
     extern __shared__ double rsm[];
     __shared__ double red[NW][3];
-    double *sC = rsm, *sw = sC + N * PITCH, *sa = sw + N * PITCH, *sb = sa + P * N;
+    double *sC = rsm, *sw = sC + N * PITCH, *sa = sw + N * PITCH, *sb = sa + P * N, *ta = sb + P * N, *tb = ta + P * N;
     const int tid = threadIdx.x, j = tid % N, c = tid / N, m = blockIdx.x;
     double *Cm = C + (size_t)m * N * N;
     for (int i = tid; i < N * N; i += NT) sC[(i / N) * PITCH + (i % N)] = Cm[i];
@@ -119,16 +148,16 @@ __global__ void __launch_bounds__(NC * NC / RES_LC) k_step2d_resident(const __gr
             ++cursor;
         }
         if (last) break;
-        __syncthreads();                     // every mu has been read: w may be overwritten
-        // ---- phase 3: y-sweep of the column (exact periodic solve, exchange slots [chunk][column])
-        chunk_solve<LC>(prm, v, sa + j, sb + j, c, N);
+        // ---- phase 3: y-sweep of the column (exact periodic solve, exchange slots [chunk][column]); its first barrier comes after
+        // every mu read above and before any write of w below
+        res_chunk_solve<LC>(prm, v, sa, sb, ta, tb, c, N, j);
 #pragma unroll
         for (int k = 0; k < LC; ++k) sw[(r0 + k) * PITCH + j] = v[k];
         __syncthreads();
         // ---- phase 4: x-sweep of row j, columns r0 .. r0 + 15, and the update
 #pragma unroll
         for (int k = 0; k < LC; ++k) v[k] = sw[j * PITCH + r0 + k];
-        chunk_solve<LC>(prm, v, sa + j, sb + j, c, N);
+        res_chunk_solve<LC>(prm, v, sa, sb, ta, tb, c, N, j);
 #pragma unroll
         for (int k = 0; k < LC; ++k) sC[j * PITCH + r0 + k] += v[k];
         __syncthreads();
@@ -152,7 +181,7 @@ __global__ void __launch_bounds__(NC * NC / RES_LC) k_step2d_resident(const __gr
 static inline size_t resident_cl_smem(int N, int CS)
 {
     const size_t rows = N / CS, nt = (size_t)N * rows / RES_LC;
-    return ((size_t)2 * rows * (N + 1) + (size_t)4 * N + 6 * nt) * 8;
+    return ((size_t)2 * rows * (N + 1) + (size_t)4 * N + 8 * nt) * 8;
 }
 
 // grid = members * CS (cluster dimension CS), block = NC * (NC / CS) / 16, dynamic smem = resident_cl_smem(NC, CS)
@@ -168,7 +197,7 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
     __shared__ double red[NW][3];
     __shared__ double cpart[CS][3];
     double *sC = rsm, *sw = sC + ROWS * PITCH, *hC = sw + ROWS * PITCH, *hM = hC + 2 * N;      // halos: [0] row above, [1] row below
-    double *yFa = hM + 2 * N, *yFb = yFa + NT, *yBa = yFb + NT, *yBb = yBa + NT, *xa = yBb + NT, *xb = xa + NT;
+    double *yFa = hM + 2 * N, *yFb = yFa + NT, *yBa = yFb + NT, *yBb = yBa + NT, *xa = yBb + NT, *xb = xa + NT, *xc = xb + NT, *xd = xc + NT;
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (int)cluster.block_rank(), prevR = (rank + CS - 1) % CS, nextR = (rank + 1) % CS;
     const int tid = threadIdx.x, m = blockIdx.x / CS;
@@ -248,8 +277,8 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
             ++cursor;
         }
         if (last) break;
-        __syncthreads();                     // every LOCAL mu read is done (the halos were pushed): w may be overwritten
-        // ---- phase 3: y-sweep, the line spread over the cluster
+        // ---- phase 3: y-sweep, the line spread over the cluster (its first cluster barrier comes after every mu read above and
+        // before any write of w below)
         {
             double a = 0.0, b = 0.0;
             v[1] = fma(np, v[0], v[1]);
@@ -293,7 +322,7 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
         // ---- phase 4: x-sweep of local row y, columns x0 .. x0 + 15, the update, and the new edge rows into the neighbours' halos
 #pragma unroll
         for (int k = 0; k < LC; ++k) v[k] = sw[y * PITCH + x0 + k];
-        chunk_solve<LC>(prm, v, xa + y, xb + y, cx, ROWS);
+        res_chunk_solve<LC>(prm, v, xa, xb, xc, xd, cx, ROWS, y);
 #pragma unroll
         for (int k = 0; k < LC; ++k) {
             const double cn = sC[y * PITCH + x0 + k] + v[k];
@@ -319,17 +348,17 @@ __global__ void __launch_bounds__(NC * (NC / CS) / RES_LC, 1) k_step2d_resident_
 // ------------------------------------------------------------------------------------------------------------------
 static inline size_t resident2_smem(int N)
 {
-    return ((size_t)4 * N * (N / 2 + 1) + (size_t)2 * (N / RES_LC) * N) * 8;
+    return ((size_t)4 * N * (N / 2 + 1) + (size_t)4 * (N / RES_LC) * N) * 8;
 }
 
-// the exact periodic solve of chunk_solve (ch_kernels.cuh) for two lines at once (shared barriers); slots [chunk][line]
+// res_chunk_solve for two lines at once (shared barriers)
 template <int LC>
-__device__ __forceinline__ void chunk_solve_pair(const SweepParams &prm, double (&u)[LC], double (&v)[LC], double *sa, double *sb,
-                                                 int c, int stride, int i1, int i2)
+__device__ __forceinline__ void chunk_solve_pair(const SweepParams &prm, double (&u)[LC], double (&v)[LC], double *fa, double *fb,
+                                                 double *ba, double *bb, int c, int stride, int i1, int i2)
 {
     const double np = prm.np, nq = prm.nq;
     const int P = prm.P;
-    auto state_in = [&](int dir, double &a1, double &b1, double &a2, double &b2) {
+    auto state_in = [&](const double *sa, const double *sb, int dir, double &a1, double &b1, double &a2, double &b2) {
         a1 = b1 = a2 = b2 = 0.0;
         int s = c;
         for (int j = 0; j < prm.K; ++j) {
@@ -347,20 +376,19 @@ __device__ __forceinline__ void chunk_solve_pair(const SweepParams &prm, double 
     u[1] = fma(np, u[0], u[1]); v[1] = fma(np, v[0], v[1]);
 #pragma unroll
     for (int k = 2; k < LC; ++k) { u[k] = fma(np, u[k - 1], fma(nq, u[k - 2], u[k])); v[k] = fma(np, v[k - 1], fma(nq, v[k - 2], v[k])); }
-    sa[c * stride + i1] = u[LC - 1]; sb[c * stride + i1] = u[LC - 2];
-    sa[c * stride + i2] = v[LC - 1]; sb[c * stride + i2] = v[LC - 2];
+    fa[c * stride + i1] = u[LC - 1]; fb[c * stride + i1] = u[LC - 2];
+    fa[c * stride + i2] = v[LC - 1]; fb[c * stride + i2] = v[LC - 2];
     __syncthreads();
-    state_in(+1, a1, b1, a2, b2);
+    state_in(fa, fb, +1, a1, b1, a2, b2);
 #pragma unroll
     for (int k = 0; k < LC; ++k) { u[k] = fma(prm.alpha[k], a1, fma(prm.beta[k], b1, u[k])); v[k] = fma(prm.alpha[k], a2, fma(prm.beta[k], b2, v[k])); }
-    __syncthreads();
     u[LC - 2] = fma(np, u[LC - 1], u[LC - 2]); v[LC - 2] = fma(np, v[LC - 1], v[LC - 2]);
 #pragma unroll
     for (int k = LC - 3; k >= 0; --k) { u[k] = fma(np, u[k + 1], fma(nq, u[k + 2], u[k])); v[k] = fma(np, v[k + 1], fma(nq, v[k + 2], v[k])); }
-    sa[c * stride + i1] = u[0]; sb[c * stride + i1] = u[1];
-    sa[c * stride + i2] = v[0]; sb[c * stride + i2] = v[1];
+    ba[c * stride + i1] = u[0]; bb[c * stride + i1] = u[1];
+    ba[c * stride + i2] = v[0]; bb[c * stride + i2] = v[1];
     __syncthreads();
-    state_in(-1, a1, b1, a2, b2);
+    state_in(ba, bb, -1, a1, b1, a2, b2);
 #pragma unroll
     for (int k = 0; k < LC; ++k) {
         u[k] = fma(prm.alpha[LC - 1 - k], a1, fma(prm.beta[LC - 1 - k], b1, u[k]));
@@ -378,7 +406,7 @@ __global__ void __launch_bounds__((NC / 2) * (NC / RES_LC), NC <= 64 ? 3 : 1) k_
     static_assert(NT % 32 == 0, "whole warps");
     extern __shared__ double rsm[];
     __shared__ double red[NG][3];
-    double *sCE = rsm, *sCO = sCE + N * PT, *swE = sCO + N * PT, *swO = swE + N * PT, *sa = swO + N * PT, *sb = sa + P * N;
+    double *sCE = rsm, *sCO = sCE + N * PT, *swE = sCO + N * PT, *swO = swE + N * PT, *sa = swO + N * PT, *sb = sa + P * N, *ta = sb + P * N, *tb = ta + P * N;
     const int tid = threadIdx.x, ih = tid % H, c = tid / H, m = blockIdx.x;
     double *Cm = C + (size_t)m * N * N;
     // row mapping: rows y1 = ih and y2 = ih + H, columns 16 c .. 16 c + 15; their C values stay in registers
@@ -465,9 +493,8 @@ __global__ void __launch_bounds__((NC / 2) * (NC / RES_LC), NC <= 64 ? 3 : 1) k_
             ++cursor;
         }
         if (last) break;
-        __syncthreads();                     // every mu has been read: w may be overwritten
-        // ---- phase 3: y-sweep of the two columns
-        chunk_solve_pair<LC>(prm, vA, vB, sa, sb, c, N, 2 * ih, 2 * ih + 1);
+        // ---- phase 3: y-sweep of the two columns (first barrier: after every mu read above, before any write of w below)
+        chunk_solve_pair<LC>(prm, vA, vB, sa, sb, ta, tb, c, N, 2 * ih, 2 * ih + 1);
 #pragma unroll
         for (int k = 0; k < LC; ++k) { swE[(r0 + k) * PT + ih] = vA[k]; swO[(r0 + k) * PT + ih] = vB[k]; }
         __syncthreads();
@@ -477,7 +504,7 @@ __global__ void __launch_bounds__((NC / 2) * (NC / RES_LC), NC <= 64 ? 3 : 1) k_
             const double *pl = (k & 1) ? swO : swE;
             vA[k] = pl[y1 * PT + (x0 + k) / 2]; vB[k] = pl[y2 * PT + (x0 + k) / 2];
         }
-        chunk_solve_pair<LC>(prm, vA, vB, sa, sb, c, N, y1, y2);
+        chunk_solve_pair<LC>(prm, vA, vB, sa, sb, ta, tb, c, N, y1, y2);
 #pragma unroll
         for (int k = 0; k < LC; ++k) {
             double *pl = (k & 1) ? sCO : sCE;
