@@ -41,7 +41,7 @@ ALGO_BYTES = {
 # flushed before the launch, so the L2 hits the live step gets from walking the ensemble up in one kernel and down in
 # the next do not show, and part of the write-back is still in L2 when the launch ends.
 # member-resident stepping: DFMA + DADD + DMUL per grid-point update (ncu, profiles/r02_ncu_full_resident.md) and the fp64 peak
-RESIDENT_FP64_INSTR_PER_UPDATE = 29.65
+RESIDENT_FP64_INSTR_PER_UPDATE = 30.1
 ALU_PEAK_TINSTR = 148 * 64 * 1.965e9 / 1e12
 
 NCU_TRAFFIC_BYTES = {
