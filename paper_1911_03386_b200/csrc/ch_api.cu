@@ -91,6 +91,7 @@ struct ch_ctx {
     bool resident_ok;
     int res_clusters;            // clusters of that size resident on the device
     int sms;                     // multiprocessors of the device
+    int opt_pdl;                 // 0: line kernel and x-sweep/update are launched as programmatic dependents, 1: plain launches
     int opt_resident;            // one-CTA kernel: 0 auto, 1 one line per thread, 2 two lines per thread
     int res_CS;                  // CTAs per member: 1 (N <= 96), else the cluster size (N = 128: 2, N = 256: 8)
     // ch_run_host: the kernels run on a member sub-range ("view"): M, total, C, w point at the view, these keep the whole
@@ -125,6 +126,20 @@ static int fuse_mode(const ch_ctx *c)
 }
 
 static bool use_rhs3_stream(const ch_ctx *c) { return c->r3_ok && c->opt_rhs3 != 1; }
+
+// Launch that may overlap the tail of the kernel before it on the stream (programmatic dependent launch; the kernel calls pdl_wait()
+// before it touches memory): option "pdl" 1 switches it off.
+template <typename... KArgs, typename... Args>
+static void pdl_launch(ch_ctx *c, void (*kernel)(KArgs...), int grid, int block, size_t smem, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = c->opt_pdl == 1 ? 0 : 1;
+    cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
 
 // member-resident stepping over clusters: (N, CTAs per member) instantiated
 // (measured on B200, updates/s at 512 / 256 members: 128^2: 2 CTAs 1.59e11, 4 CTAs 1.41e11, 8 CTAs 1.44e11; 256^2: 8 CTAs 1.13e11, 16 CTAs 1.14e11)
@@ -414,7 +429,7 @@ extern "C" int ch_create(ch_ctx **out, int ensemble, int N, int D, double gamma,
         }
     }
     // member-resident stepping: the member and its work array in one CTA's shared memory
-    c->resident_ok = false; c->res_CS = 1; c->sms = 1; c->opt_resident = 0;
+    c->resident_ok = false; c->res_CS = 1; c->sms = 1; c->opt_resident = 0; c->opt_pdl = 0;
     if (D == 2 && c->LC == RES_LC && (N == 128 || N == 256)) {
         c->res_CS = N == 128 ? 2 : 8;
         int nclusters = 0;
@@ -651,6 +666,11 @@ extern "C" int ch_set_option(ch_ctx *ctx, const char *key, int value)
         ctx->opt_linesync = value;
         return CH_OK;
     }
+    if (!strcmp(key, "pdl")) {
+        if (value < 0 || value > 1) return fail(ctx, CH_EINVAL, "ch_set_option: pdl must be 0 (programmatic dependent launches) or 1 (plain launches)");
+        ctx->opt_pdl = value;
+        return CH_OK;
+    }
     if (!strcmp(key, "resident_lines")) {
         if (value < 0 || value > 2) return fail(ctx, CH_EINVAL, "ch_set_option: resident_lines must be 0 (auto), 1 (one line per thread) or 2 (two lines per thread)");
         ctx->opt_resident = value;
@@ -691,6 +711,7 @@ extern "C" int ch_get_option(const ch_ctx *ctx, const char *key, int *value)
     if (!strcmp(key, "local_reach")) { *value = ctx->loc_H; return CH_OK; }
     if (!strcmp(key, "resident")) { *value = ctx->resident_ok ? ctx->res_CS : 0; return CH_OK; }
     if (!strcmp(key, "resident_lines")) { *value = ctx->opt_resident; return CH_OK; }
+    if (!strcmp(key, "pdl")) { *value = ctx->opt_pdl; return CH_OK; }
     if (!strcmp(key, "resident_clusters")) { *value = ctx->resident_ok ? ctx->res_clusters : 0; return CH_OK; }
     return CH_EINVAL;
 }
@@ -923,8 +944,8 @@ static void launch_rhs_sweep_y_line(ch_ctx *c, bool diag, bool write)
     if (c->N == NC) {                                                                                               \
         if (diag && nb) k_rhs_sweep_y_line<NC, true, true><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
         else if (diag) k_rhs_sweep_y_line<NC, true, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
-        else if (nb) k_rhs_sweep_y_line<NC, false, true><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials); \
-        else k_rhs_sweep_y_line<NC, false, false><<<grid, NC, smem, c->stream>>>(p, c->C, c->w, c->partials);       \
+        else if (nb) pdl_launch(c, k_rhs_sweep_y_line<NC, false, true>, grid, NC, smem, p, (const double *)c->C, c->w, c->partials); \
+        else pdl_launch(c, k_rhs_sweep_y_line<NC, false, false>, grid, NC, smem, p, (const double *)c->C, c->w, c->partials);       \
     }
     LINE_SIZES(X)
 #undef X
@@ -1032,8 +1053,8 @@ static void launch_sweep_x_update(ch_ctx *c, bool unscaled)
     threads = LPB * P;
     const int blocks = (int)((total_lines + LPB - 1) / LPB);
     const size_t smem = (size_t)2 * LPB * N * 8 + (size_t)2 * LPB * P * 8;
-    if (LC == 16) k_sweep_x_update<16><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
-    else k_sweep_x_update<32><<<blocks, threads, smem, c->stream>>>(prm, c->w, c->C, N, total_lines, LPB);
+    if (LC == 16) pdl_launch(c, k_sweep_x_update<16>, blocks, threads, smem, prm, (const double *)c->w, c->C, N, total_lines, LPB);
+    else pdl_launch(c, k_sweep_x_update<32>, blocks, threads, smem, prm, (const double *)c->w, c->C, N, total_lines, LPB);
 }
 
 // the whole 2D step in one pass (ch_local2d.cuh): reads c->C, writes c->w, then the two arrays swap roles
@@ -1166,7 +1187,7 @@ static bool graph_wanted(const ch_ctx *c)
 
 static bool ensure_graph(ch_ctx *c)
 {
-    const long long sig = ((((((long long)c->opt_sweep * 8 + c->opt_fuse) * 4 + c->opt_linesync) * 4 + c->opt_scan) * 4 + c->opt_rhs3) * 4
+    const long long sig = ((((((long long)(c->opt_sweep * 2 + c->opt_pdl) * 8 + c->opt_fuse) * 4 + c->opt_linesync) * 4 + c->opt_scan) * 4 + c->opt_rhs3) * 4
                            + c->opt_sweep3);
     if (c->gexec && c->gsig == sig) return true;
     if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }

@@ -259,6 +259,8 @@ __global__ void k_sweep_x_update(const __grid_constant__ SweepParams prm, const 
     double *sb = sa + LPB * P;
 
     const unsigned long long pol = l2_evict_first_policy();     // w is dead after this read; C is overwritten below
+    pdl_trigger();
+    pdl_wait();
     for (int g = t; g < G; g += nthreads) line_cp_async16_hint(&sl[swz<LC>(g)], gw + g, pol);
     cp_async_commit();
     for (int g = t; g < G; g += nthreads) line_cp_async16_hint(&sC[g], gC + g, pol);
