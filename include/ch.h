@@ -173,7 +173,7 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *   "resident_lines" one-CTA member-resident kernel (N <= 96): 0 auto (two lines per thread when at least two CTAs share an SM, i.e.
  *              ensemble >= 2 x multiprocessors, or N = 96), 1 one line per thread, 2 two lines per thread (half the shared-
  *              memory traffic, half the warps); fields and samples are bitwise the same either way
- *   "pdl"      0 (default): the line kernel and the x-sweep/update kernel are launched as programmatic dependents (they may start
+ *   "pdl"      0 (default): the stepping kernels of the fast paths are launched as programmatic dependents (they may start
  *              while their predecessor on the stream drains and wait inside the kernel before touching memory; same results),
  *              1 plain launches
  *   "linesync" line kernel: 0 auto (neighbour-warp flags when the closure is truncated to 2 chunks), 1 CTA barriers

@@ -130,10 +130,10 @@ static bool use_rhs3_stream(const ch_ctx *c) { return c->r3_ok && c->opt_rhs3 !=
 // Launch that may overlap the tail of the kernel before it on the stream (programmatic dependent launch; the kernel calls pdl_wait()
 // before it touches memory): option "pdl" 1 switches it off.
 template <typename... KArgs, typename... Args>
-static void pdl_launch(ch_ctx *c, void (*kernel)(KArgs...), int grid, int block, size_t smem, Args... args)
+static void pdl_launch(ch_ctx *c, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args)
 {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -732,9 +732,9 @@ static void launch_rhs_t(ch_ctx *c, const double *C, double *r, double scale)
         p.nunits = c->r3_parts * c->M; p.write = WRITE ? 1 : 0; p.rev = c->dir3;
         const int grid = p.nunits < c->r3_resident ? p.nunits : c->r3_resident;
         const size_t smem = rhs3_stream_smem(c->N);
-        if (c->N == 64) k_rhs3d_stream<64, DIAG><<<grid, 256, smem, c->stream>>>(p, C, r, c->partials);
-        else if (c->N == 96) k_rhs3d_stream<96, DIAG><<<grid, 384, smem, c->stream>>>(p, C, r, c->partials);
-        else k_rhs3d_stream<128, DIAG><<<grid, 512, smem, c->stream>>>(p, C, r, c->partials);
+        if (c->N == 64) pdl_launch(c, k_rhs3d_stream<64, DIAG>, grid, 256, smem, p, C, r, c->partials);
+        else if (c->N == 96) pdl_launch(c, k_rhs3d_stream<96, DIAG>, grid, 384, smem, p, C, r, c->partials);
+        else pdl_launch(c, k_rhs3d_stream<128, DIAG>, grid, 512, smem, p, C, r, c->partials);
         return;
     }
     if (c->D == 2) {
@@ -858,9 +858,9 @@ static void launch_sweep(ch_ctx *c, double *w, int axis, bool update, bool scale
     const size_t smem = (size_t)2 * P * cols * 8;
 #define LAUNCH_STRIDED(LCV)                                                                                                          \
     do {                                                                                                                             \
-        if (update) k_sweep_strided<LCV, true, false><<<blocks, block, smem, c->stream>>>(prm, w, c->C, outer_stride, line_stride, inner_blocks); \
-        else if (scale) k_sweep_strided<LCV, false, true><<<blocks, block, smem, c->stream>>>(prm, w, c->C, outer_stride, line_stride, inner_blocks); \
-        else k_sweep_strided<LCV, false, false><<<blocks, block, smem, c->stream>>>(prm, w, c->C, outer_stride, line_stride, inner_blocks); \
+        if (update) pdl_launch(c, k_sweep_strided<LCV, true, false>, blocks, block, smem, prm, w, c->C, outer_stride, line_stride, inner_blocks); \
+        else if (scale) pdl_launch(c, k_sweep_strided<LCV, false, true>, blocks, block, smem, prm, w, c->C, outer_stride, line_stride, inner_blocks); \
+        else pdl_launch(c, k_sweep_strided<LCV, false, false>, blocks, block, smem, prm, w, c->C, outer_stride, line_stride, inner_blocks); \
     } while (0)
     if (LC == 16) LAUNCH_STRIDED(16); else LAUNCH_STRIDED(32);
 #undef LAUNCH_STRIDED
@@ -882,16 +882,18 @@ static void launch_sweep_xy(ch_ctx *c, double *w, int rev)
     const int N = c->N;
     const size_t smem = (size_t)N * N * 8 + (size_t)2 * P * N * 8;
     const unsigned planes = (unsigned)((size_t)c->M * N);
-    if (N == 64) { k_sweep_xy_plane<64><<<planes, 256, smem, c->stream>>>(prm, w); return; }
-    if (c->opt_sweep3 == 2) { k_sweep_xy_plane<128><<<planes, 1024, smem, c->stream>>>(prm, w); return; }
+    if (N == 64) { pdl_launch(c, k_sweep_xy_plane<64>, planes, 256, smem, prm, w); return; }
+    if (c->opt_sweep3 == 2) { pdl_launch(c, k_sweep_xy_plane<128>, planes, 1024, smem, prm, w); return; }
     // N = 128: half a plane per CTA, clusters of 2 (two CTAs of different planes per SM overlap load and compute)
     cudaLaunchConfig_t cfg = {};
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.gridDim = dim3(2 * planes); cfg.blockDim = dim3(512);
     cfg.dynamicSmemBytes = (size_t)64 * 128 * 8 + (size_t)2 * 2 * 8 * 128 * 8;
-    cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = 1;
+    cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = c->opt_pdl == 1 ? 1 : 2;
     cudaLaunchKernelEx(&cfg, k_sweep_xy_pair, prm, w);
 }
 
@@ -967,11 +969,13 @@ static void launch_rhs_sweep_y_cline(ch_ctx *c)
     p.ntiles = c->cl_strips * c->M; p.write = 1;
     const int ncl = p.ntiles < c->cl_resident ? p.ntiles : c->cl_resident;
     cudaLaunchConfig_t cfg = {};
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = c->cl_CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.gridDim = dim3(c->cl_CS * ncl); cfg.blockDim = dim3(CLINE_NC); cfg.dynamicSmemBytes = cline_smem();
-    cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = 1;
+    cfg.stream = c->stream; cfg.attrs = at; cfg.numAttrs = c->opt_pdl == 1 ? 1 : 2;
 #define X(CSV)                                                                                                     \
     if (c->cl_CS == CSV) {                                                                                          \
         if (scan) cudaLaunchKernelEx(&cfg, k_rhs_sweep_y_cline<CSV, true>, p, (const double *)c->C, c->w);          \
@@ -1083,7 +1087,7 @@ static void launch_step_local(ch_ctx *c)
     if (grid < 1) grid = 1;
     p.span = (p.total_rows + grid - 1) / grid;
     grid = (p.total_rows + p.span - 1) / p.span;
-    k_step2d_local<<<(unsigned)grid, LOC_NT, local_smem_bytes(), c->stream>>>(p, c->C, c->w);
+    pdl_launch(c, k_step2d_local, (unsigned)grid, LOC_NT, local_smem_bytes(), p, (const double *)c->C, c->w);
     double *t = c->C; c->C = c->w; c->w = t;
 }
 

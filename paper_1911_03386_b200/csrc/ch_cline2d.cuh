@@ -169,7 +169,9 @@ __global__ void __launch_bounds__(CLINE_NC, 1) k_rhs_sweep_y_cline(const __grid_
     if (tid < NW) { flagF[tid] = 0; flagB[tid] = 0; }
     if (tid == 0) { gflagF = 0; gflagB = 0; }
     __syncthreads();
+    pdl_trigger();
     cl_sync_all();                 // every CTA of the cluster has initialised its flags before anyone pushes
+    pdl_wait();
     // where the boundary warps push their chunk states: ghost slots and ghost flag of the neighbouring CTA
     unsigned remSlot = 0, remFlag = 0;
     if (wid == NW - 1) {

@@ -40,6 +40,13 @@ __device__ __forceinline__ void ck_cp_async_wait_all()
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
 }
 
+// Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start while the
+// kernel before it on the stream is still running; pdl_wait() blocks until that kernel has completed and its writes are visible
+// (it must come before the first access to anything the predecessor touches), pdl_trigger() lets the NEXT kernel's CTAs be
+// scheduled as soon as every CTA of this one has started.  Both are no-ops in a kernel launched the plain way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
+
 // ------------------------------------------------------------------------------------
 // reductions
 // ------------------------------------------------------------------------------------
@@ -382,6 +389,8 @@ __global__ void __launch_bounds__(512) k_sweep_strided(const __grid_constant__ S
                                 double *__restrict__ C, size_t outer_stride, size_t line_stride, int inner_blocks)
 {
     extern __shared__ double sx[];
+    pdl_trigger();
+    pdl_wait();
     const int COLS = blockDim.x, P = blockDim.y;
     const int tx = threadIdx.x, c = threadIdx.y;
     const unsigned bid = prm.rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
@@ -555,6 +564,8 @@ __global__ void __launch_bounds__(256) k_sweep_pcr_x(const __grid_constant__ Pcr
 template <int NC>
 __global__ void __launch_bounds__(NC * NC / 16, NC == 64 ? 3 : 1) k_sweep_xy_plane(const __grid_constant__ SweepParams prm, double *__restrict__ w)
 {
+    pdl_trigger();
+    pdl_wait();
     constexpr int LC = 16, P = NC / LC, NT = NC * NC / LC, G = NC * NC / 2;
     extern __shared__ double2 sl[];
     double *sx = reinterpret_cast<double *>(sl + G);
@@ -619,6 +630,8 @@ __global__ void __launch_bounds__(512, 2) k_sweep_xy_pair(const __grid_constant_
     unsigned rank;
     asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(rank));
     const unsigned peer = rank ^ 1u;
+    pdl_trigger();
+    pdl_wait();
     const size_t plane = prm.rev ? (gridDim.x >> 1) - 1 - (blockIdx.x >> 1) : (blockIdx.x >> 1);
     double *wp = w + plane * NC * NC + (size_t)rank * HR * NC;
     double2 *g2 = reinterpret_cast<double2 *>(wp);

@@ -59,13 +59,6 @@ __device__ __forceinline__ void line_cp_async16_hint(void *smem_dst, const void 
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gsrc), "l"(policy) : "memory");
 }
-// Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start while the
-// kernel before it on the stream is still running; pdl_wait() blocks until that kernel has completed and its writes are visible
-// (it must come before the first access to anything the predecessor touches), pdl_trigger() lets the NEXT kernel's CTAs be
-// scheduled as soon as every CTA of this one has started.  Both are no-ops in a kernel launched the plain way.
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
-__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
-
 __device__ __forceinline__ void line_cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void line_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 

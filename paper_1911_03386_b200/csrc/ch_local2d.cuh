@@ -36,6 +36,8 @@
 
 #include <type_traits>
 
+#include "ch_kernels.cuh"     // pdl_wait / pdl_trigger
+
 #define LOC_NW 7                          // warps per CTA
 #define LOC_NT (32 * LOC_NW)
 #define LOC_LB 32                         // rows per block
@@ -113,6 +115,8 @@ __global__ void __launch_bounds__(LOC_NT, 2) k_step2d_local(const __grid_constan
     double *const stage = zring + LOC_ZRING;                              // [LOC_NW][LOC_SR][LOC_WC]
     double2 *const side = reinterpret_cast<double2 *>(stage + LOC_STAGE); // [2][LOC_NW + 1][LOC_LB]
     const int tid = threadIdx.x, lane = tid & 31;
+    pdl_trigger();
+    pdl_wait();
     const int wid = __shfl_sync(0xffffffffu, tid >> 5, 0);     // warp-uniform for the compiler: loader addresses stay in uniform registers
     const int N = prm.N, H = prm.H, He = (H + 1) & ~1;
     const double np = prm.np, nq = prm.nq, mgam = prm.mgam, k1 = prm.k1;

@@ -53,6 +53,8 @@ __global__ void __launch_bounds__(4 * NC, 1) k_rhs3d_stream(const __grid_constan
     __shared__ double red[16][3];
     const int tid = threadIdx.x, li = tid & 15, hw = tid >> 4;
     const int hwm = (hw + NHW - 1) % NHW, hwp = (hw + 1) % NHW;
+    pdl_trigger();
+    pdl_wait();
     double2 *stage = sm2 + tid;                                   // plane slot p, row j: stage[(p * RY + j) * NT]
     // published edge rows: [parity][top|bottom][half-warp][lane]
     double2 *exC = sm2 + (size_t)3 * RY * NT, *exM = exC + 2 * 2 * NHW * 16;
