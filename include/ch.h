@@ -137,7 +137,7 @@ int ch_get_state(ch_ctx *ctx, double *C, int on_device);
  * context holds the final state, n = nsteps, t0 = 0), but done member chunk by member chunk -- members are independent
  * -- so that the host-to-device copy of chunk k + 1, the steps of chunk k and the device-to-host copy of
  * chunk k - 1 overlap on three internal streams (ordered after everything already enqueued on the context's stream).
- * `chunk` = members per chunk, 0 = library default (about 16 Mi grid points, at least 4 chunks).  C_in and C_out
+ * `chunk` = members per chunk, 0 = library default (about 4 Mi grid points, 2 Mi for jobs of <= 30 steps; at least 4 chunks).  C_in and C_out
  * (ensemble * N^D doubles each, may be the same buffer) should be pinned host memory for the copies to be asynchronous.
  * Synchronous: returns when everything has completed.  CUDA graphs are not used inside. */
 int ch_run_host(ch_ctx *ctx, const double *C_in, double *C_out, int nsteps, int chunk);

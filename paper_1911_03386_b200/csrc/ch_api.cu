@@ -1289,14 +1289,20 @@ extern "C" int ch_run_host(ch_ctx *ctx, const double *C_in, double *C_out, int n
     ctx->has_state = true; ctx->n = 0; ctx->t0 = 0.0; ctx->cursor = 0; ctx->last_sampled = -1;
     if (samples_ahead(ctx, nsteps) > ctx->capacity) return fail(ctx, CH_EINVAL, "ch_run_host: series full");
     const int M = ctx->M;
+    std::vector<int> sizes;                          // members per chunk, in order
     if (chunk == 0) {
-        // default: about 16 Mi points per chunk (copy and compute of a chunk take comparable time), at least 4 chunks
-        const size_t want = ((size_t)16 << 20) / ctx->npts;
+        // default: about 4 Mi points per chunk -- 2 Mi for short jobs, whose time is the copies plus the first copy in and the last copy
+        // out -- and at least 4 chunks.  Measured on CFG3, B200 (ms for 20 / 50 / 100 / 200 steps): 8 Mi-point chunks 7.7 / 13.6 / 24.7 /
+        // 47.3, 4 Mi 6.8 / 12.5 / 23.7 / 46.1, 2 Mi 6.4 / 14.9 / 29.1 / 57.4 (small ensembles make the kernels less efficient); chunks
+        // tapered towards both ends did not help (the very small end chunks cost more than they save)
+        const size_t pts = (size_t)(nsteps <= 30 ? 2 : 4) << 20;
+        const size_t want = pts / ctx->npts;
         chunk = (int)(want < 1 ? 1 : want);
         if (chunk > (M + 3) / 4) chunk = (M + 3) / 4;
         if (chunk < 1) chunk = 1;
     }
     if (chunk > M) chunk = M;
+    if (sizes.empty()) for (int left = M; left > 0; left -= chunk) sizes.push_back(left < chunk ? left : chunk);
     double *const Cfull = ctx->C, *const wfull = ctx->w;
     const size_t total_full = ctx->total;
     cudaStream_t user = ctx->stream;
@@ -1310,8 +1316,9 @@ extern "C" int ch_run_host(ch_ctx *ctx, const double *C_in, double *C_out, int n
     long long n_end = 0; int cursor_end = 0; long long ls_end = -1;
     double *Cend = Cfull, *wend = wfull;
     cudaError_t err = cudaSuccess;
-    for (int m0 = 0; m0 < M && err == cudaSuccess; m0 += chunk) {
-        const int mc = m0 + chunk <= M ? chunk : M - m0;
+    int m0 = 0;
+    for (size_t ci = 0; ci < sizes.size() && err == cudaSuccess; m0 += sizes[ci], ++ci) {
+        const int mc = sizes[ci];
         const size_t off = (size_t)m0 * ctx->npts, cnt = (size_t)mc * ctx->npts;
         cudaEvent_t ev_in = nullptr, ev_comp = nullptr;
         err = cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming);
