@@ -179,8 +179,8 @@ int ch_sweep(ch_ctx *ctx, double *w, int axis, int on_device);
  *   "linesync" line kernel: 0 auto (neighbour-warp flags when the closure is truncated to 2 chunks), 1 CTA barriers
  *   "scan"     closure of the chunk states: 0 auto (log-depth shuffle scan when the K-term sum is long), 1 K-term
  *              sum always, 2 scan wherever it is available
- *   "graph"    0 auto (ensembles of <= 8 Mi points, which are launch bound, replay a CUDA graph of 8 plain steps
- *              between sampling steps; bitwise the same results and launch count), 1 plain launches, 2 graphs always
+ *   "graph"    0 auto = 2 (plain steps between sampling steps are replayed as a CUDA graph of 8 steps, captured on first use;
+ *              bitwise the same results and launch count; not while profiling), 1 plain launches, 2 graphs always
  *   "rhs3"     3D RHS: 0 auto (z-marching kernel for N in {64, 128}), 1 tile kernel
  *   "sweep3"   3D x/y sweeps: 0 auto (one pass per z-plane in shared memory for N in {64, 128}; cluster pairs at
  *              N = 128), 1 separate x- and y-sweeps, 2 one CTA per plane

@@ -1186,7 +1186,8 @@ static void launch_one_step(ch_ctx *ctx, bool sample)
 static bool graph_wanted(const ch_ctx *c)
 {
     if (c->opt_graph == 1 || c->graph_broken || c->profiling) return false;
-    return c->opt_graph == 2 || c->total <= ((size_t)8 << 20);
+    // every size: launch-bound ensembles gain most (CFG1-like: 2x), but the large configs still gain 0.3 - 1.3 % (CFG3 0.2265 -> 0.2236 ms median)
+    return true;
 }
 
 static bool ensure_graph(ch_ctx *c)
